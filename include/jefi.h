@@ -1,0 +1,147 @@
+/*
+ * jefi.h -- C ABI of the B200 (sm_100a) library that evaluates the discretised Jefimenko
+ * retarded-time sums for E(r,t) and B(r,t) (arxiv 2104.05426, "JefiGPU").
+ *
+ * What the library computes (Sec. 2.2 Eq. (4)-(6); readings Q1-Q8 of
+ * DESIGN.md), per observation point r and evaluation step n (t = t0 + n*dt):
+ *
+ *   E(r,t) = dV/(4 pi) * sum_cells [ d*( rho/R^3 + rho_dot/(c R^2) ) - J_dot/(c^2 R) ]
+ *   B(r,t) = dV/(4 pi) * sum_cells [ ( J/R^3 + J_dot/(c R^2) ) x d ]
+ *
+ *   d = r - r'_cell, R = |d|; rho, J, rho_dot, J_dot of that cell at the stored step
+ *   m = n - floor(R/(c dt) + 0.5)  (Eq. (6): t_r = t - R/c, nearest stored snapshot);
+ *   m < 0 contributes zero (the paper's sources vanish before t0);
+ *   cells with R < 0.5*min(dx,dy,dz) are skipped (coarse screening);
+ *   dV = dx*dy*dz of the source grid.
+ *
+ * Every step of that path runs in hand-written CUDA kernels; there is no CPU fallback and
+ * no other backend.  All pointers named *_dev are DEVICE pointers of the context's dtype,
+ * all pointers named *_host are HOST pointers; nothing here is a torch type.  Calls are
+ * asynchronous on the given stream unless stated; one context must not be used from two
+ * streams at the same time.  Errors are return codes only (nothing is thrown, nothing
+ * aborts); argument errors are detected before any launch.
+ */
+#ifndef JEFI_H
+#define JEFI_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct jefi_ctx jefi_ctx;          /* opaque; owned by the library */
+typedef void* jefi_stream;                 /* a cudaStream_t (0 = legacy default stream) */
+
+typedef enum {
+    JEFI_OK = 0,
+    JEFI_ERR_INVALID_ARG = 1,              /* null pointer, n <= 0, dt <= 0, c <= 0, bad range */
+    JEFI_ERR_CUDA = 2,                     /* a CUDA runtime call or launch failed; see jefi_last_error */
+    JEFI_ERR_OOM = 3,                      /* device allocation failed */
+    JEFI_ERR_NO_HISTORY = 4,               /* jefi_fields before jefi_upload_history */
+    JEFI_ERR_TIME_RANGE = 5,               /* step outside [0, nsteps-1] or t off the step grid */
+    JEFI_ERR_UNSUPPORTED = 6               /* valid request this build does not implement */
+} jefi_status;
+
+typedef enum { JEFI_F32 = 0, JEFI_F64 = 1 } jefi_dtype;
+
+/* A regular grid (source and observational regions each have their own sizes
+ * and spacings and need not overlap).  origin = CENTRE of cell/point (0,0,0) (PAPER.md:137:
+ * 15 cells x 0.4 span [-3,3], so samples are cell centres); index order x fastest:
+ * linear index j = (k_z*n[1] + j_y)*n[0] + i_x.  All host fp64. */
+typedef struct {
+    int32_t n[3];
+    double  origin[3];
+    double  spacing[3];
+} jefi_grid_desc;
+
+/* Observation set.  kind 0: the regular grid `grid` (the paper's case).  kind 1: an explicit
+ * list of `npoints` positions, points_dev[npoints][3] of the context dtype, device memory
+ * owned by the caller and read at every jefi_fields call. */
+typedef struct {
+    int32_t        kind;
+    jefi_grid_desc grid;
+    int64_t        npoints;
+    const void*    points_dev;
+} jefi_obs_desc;
+
+/* Stored history: nsteps snapshots m = 0..nsteps-1 at times t0 + m*dt (PAPER.md:231:
+ * rho_GPU -> [rho_0 ... rho_lts]).  deriv_mode 0: centred time difference inside the stored
+ * history, one-sided at both ends (BASELINE.json north_star (b)); 1: the paper's backward
+ * difference (f(t_r) - f(t_r - dt))/dt with f = 0 before step 0.
+ * past_mode must be 0 (zero before step 0). */
+typedef struct {
+    double  t0, dt, c;
+    int32_t nsteps;
+    int32_t deriv_mode;
+    int32_t past_mode;
+} jefi_time_desc;
+
+/* Validates the descriptors, selects `device`, and allocates everything the context will
+ * ever need on it: the packed history (2 x 16-byte (fp32) / 2 x 32-byte (fp64) half-records
+ * per (cell, step), plus one all-zero step for m < 0), partial-sum scratch, and the device
+ * output staging used by jefi_fields_host.  No kernel is launched.  *out is written only on
+ * success.  Synchronous. */
+jefi_status jefi_create(const jefi_grid_desc* src, const jefi_obs_desc* obs,
+                        const jefi_time_desc* time, jefi_dtype dtype, int device,
+                        jefi_ctx** out);
+
+/* Step a1 (pre-pass): reads rho_dev[nsteps][N_s] and J_dev[nsteps][3][N_s] (component planes;
+ * the paper's four scalar fields rho, Jx, Jy, Jz), builds d(rho)/dt and dJ/dt and
+ * writes the packed records.  The caller may free rho_dev/J_dev once `stream` has passed this
+ * call.  May be called again to replace the history. */
+jefi_status jefi_upload_history(jefi_ctx* ctx, const void* rho_dev, const void* J_dev,
+                                jefi_stream stream);
+
+/* Same, from HOST buffers (pinned for a truly asynchronous copy): copies them into a raw
+ * device staging area owned by the context (allocated on first use) and runs the pre-pass. */
+jefi_status jefi_upload_history_host(jefi_ctx* ctx, const void* rho_host, const void* J_host,
+                                     jefi_stream stream);
+
+/* Steps a2-a6: E and B at evaluation step `step` (t = t0 + step*dt) for the observation
+ * points obs_begin .. obs_begin+obs_count-1 (linear indices into the observation set).
+ * E_out_dev / B_out_dev are [3][obs_count] component planes of the context dtype, owned by
+ * the caller, fully overwritten, never accumulated into.  obs_count = 0 is a no-op. */
+jefi_status jefi_fields(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t obs_count,
+                        void* E_out_dev, void* B_out_dev, jefi_stream stream);
+
+/* Same for a time t that must lie on the step grid to within 1e-6*dt (the paper
+ * evaluates at snapshots only), else JEFI_ERR_TIME_RANGE. */
+jefi_status jefi_fields_at_time(jefi_ctx* ctx, double t, int64_t obs_begin, int64_t obs_count,
+                                void* E_out_dev, void* B_out_dev, jefi_stream stream);
+
+/* Same as jefi_fields, results copied to HOST buffers [3][obs_count] on `stream` (the paper
+ * copies E, B to the host every step).  Returns after enqueueing; synchronise the
+ * stream before reading. */
+jefi_status jefi_fields_host(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t obs_count,
+                             void* E_out_host, void* B_out_host, jefi_stream stream);
+
+/* Kernel selection for jefi_fields: 0 = automatic (tiled kernel for regular observation
+ * grids, per-point kernel otherwise), 1 = always the per-point kernel (one thread per
+ * observation point, the paper's shape PAPER.md:93), 2 = tiled kernel or JEFI_ERR_UNSUPPORTED. */
+jefi_status jefi_set_kernel(jefi_ctx* ctx, int32_t which);
+
+/* Number of kernels launched by this context so far (for the bench's launch count). */
+int64_t     jefi_launch_count(const jefi_ctx* ctx);
+
+/* Bytes of device memory owned by the context. */
+int64_t     jefi_device_bytes(const jefi_ctx* ctx);
+
+/* Waits for all work of the context's device; frees everything it owns. */
+jefi_status jefi_destroy(jefi_ctx* ctx);
+
+const char* jefi_status_string(jefi_status s);
+/* Text of the last error of this context ("" if none); valid until the next call on it. */
+const char* jefi_last_error(const jefi_ctx* ctx);
+/* The fixed nominal operation count per (observation point, source cell) interaction: 52,
+ * the flop count of the oracle's loop body. */
+int         jefi_flops_per_pair(void);
+
+/* Register-only FFMA (dtype F32) or DFMA (dtype F64) chain on `device`: returns the measured
+ * TFLOP/s in *tflops (synchronous; used by the bench to state the ALU peak it divides by). */
+jefi_status jefi_measure_alu_peak(int device, jefi_dtype dtype, double* tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* JEFI_H */

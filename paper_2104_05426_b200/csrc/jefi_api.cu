@@ -1,0 +1,320 @@
+// jefi_api.cu -- the C ABI of include/jefi.h: context, validation, error reporting, launches.
+// No arithmetic of the method lives here; every step of the path is a kernel in prepass.cu,
+// pairwise_tiled.cu and pairwise_point.cu.  There is no CPU fallback.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+#include <new>
+#include "jefi_internal.h"
+
+struct jefi_ctx {
+    jefi::Params P;
+    jefi_dtype   dtype;
+    int          device;
+    double       t0;
+    int          sm_count;
+    size_t       elem;             // sizeof(float|double)
+    void*        hist;             // packed history, [N_s][2][Tp] vec4
+    size_t       hist_bytes;
+    void*        scratch;          // partial sums (double)
+    long long    scratch_elems;
+    void*        stage_E;          // device staging for jefi_fields_host, [3][N_o]
+    void*        stage_B;
+    void*        raw_rho;          // device staging for jefi_upload_history_host (lazy)
+    void*        raw_J;
+    bool         has_history;
+    int          kernel_choice;
+    long long    launches;
+    long long    dev_bytes;
+    char         err[512];
+};
+
+namespace {
+
+void set_err(jefi_ctx* c, const char* what, cudaError_t e)
+{
+    if (!c) return;
+    if (e != cudaSuccess) snprintf(c->err, sizeof(c->err), "%s: %s", what, cudaGetErrorString(e));
+    else snprintf(c->err, sizeof(c->err), "%s", what);
+}
+
+jefi_status cuda_fail(jefi_ctx* c, const char* what, cudaError_t e)
+{
+    set_err(c, what, e);
+    cudaGetLastError();            // clear the sticky-less error state
+    return e == cudaErrorMemoryAllocation ? JEFI_ERR_OOM : JEFI_ERR_CUDA;
+}
+
+bool grid_ok(const jefi_grid_desc& g)
+{
+    for (int a = 0; a < 3; ++a) {
+        if (g.n[a] <= 0) return false;
+        if (!(g.spacing[a] > 0.0) || !isfinite(g.spacing[a]) || !isfinite(g.origin[a])) return false;
+    }
+    return true;
+}
+
+jefi_status dev_alloc(jefi_ctx* c, void** p, size_t bytes, const char* what)
+{
+    if (bytes == 0) bytes = 16;
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) { *p = nullptr; return cuda_fail(c, what, e); }
+    c->dev_bytes += (long long)bytes;
+    return JEFI_OK;
+}
+
+void free_all(jefi_ctx* c)
+{
+    cudaFree(c->hist); cudaFree(c->scratch); cudaFree(c->stage_E); cudaFree(c->stage_B);
+    cudaFree(c->raw_rho); cudaFree(c->raw_J);
+}
+
+jefi_status check_fields_args(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t obs_count,
+                              const void* E, const void* B)
+{
+    if (!ctx) return JEFI_ERR_INVALID_ARG;
+    ctx->err[0] = 0;
+    if (obs_begin < 0 || obs_count < 0 || obs_begin + obs_count > ctx->P.n_obs) {
+        set_err(ctx, "observation range outside the observation set", cudaSuccess);
+        return JEFI_ERR_INVALID_ARG;
+    }
+    if (obs_count > 0 && (!E || !B)) {
+        set_err(ctx, "null output pointer", cudaSuccess);
+        return JEFI_ERR_INVALID_ARG;
+    }
+    if (step < 0 || step >= ctx->P.T) {
+        set_err(ctx, "step outside the stored history", cudaSuccess);
+        return JEFI_ERR_TIME_RANGE;
+    }
+    if (!ctx->has_history) {
+        set_err(ctx, "jefi_fields before jefi_upload_history", cudaSuccess);
+        return JEFI_ERR_NO_HISTORY;
+    }
+    return JEFI_OK;
+}
+
+jefi_status run_fields(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t obs_count,
+                       void* E, void* B, cudaStream_t stream)
+{
+    if (obs_count == 0) return JEFI_OK;
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e != cudaSuccess) return cuda_fail(ctx, "cudaSetDevice", e);
+    jefi::FieldsLaunch L;
+    L.step = step; L.obs_begin = obs_begin; L.obs_count = obs_count;
+    L.E_out = E; L.B_out = B;
+    L.scratch = ctx->scratch; L.scratch_elems = ctx->scratch_elems;
+    L.sm_count = ctx->sm_count; L.stream = stream;
+    int n = 0;
+    if (ctx->kernel_choice != 1) {
+        n = jefi::launch_fields_tiled(ctx->P, ctx->dtype, ctx->hist, L);
+        if (n == 0 && ctx->kernel_choice == 2) {
+            set_err(ctx, "tiled kernel does not support this request", cudaSuccess);
+            return JEFI_ERR_UNSUPPORTED;
+        }
+    }
+    if (n == 0) n = jefi::launch_fields_point(ctx->P, ctx->dtype, ctx->hist, L);
+    if (n < 0) return cuda_fail(ctx, "fields kernel launch", cudaGetLastError());
+    ctx->launches += n;
+    return JEFI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+jefi_status jefi_create(const jefi_grid_desc* src, const jefi_obs_desc* obs,
+                        const jefi_time_desc* time, jefi_dtype dtype, int device, jefi_ctx** out)
+{
+    if (!src || !obs || !time || !out) return JEFI_ERR_INVALID_ARG;
+    if (dtype != JEFI_F32 && dtype != JEFI_F64) return JEFI_ERR_INVALID_ARG;
+    if (!grid_ok(*src)) return JEFI_ERR_INVALID_ARG;
+    if (obs->kind != 0 && obs->kind != 1) return JEFI_ERR_INVALID_ARG;
+    if (obs->kind == 0 && !grid_ok(obs->grid)) return JEFI_ERR_INVALID_ARG;
+    if (obs->kind == 1 && (obs->npoints < 0 || (obs->npoints > 0 && !obs->points_dev)))
+        return JEFI_ERR_INVALID_ARG;
+    if (!(time->dt > 0.0) || !(time->c > 0.0) || !isfinite(time->dt) || !isfinite(time->c) ||
+        !isfinite(time->t0) || time->nsteps <= 0)
+        return JEFI_ERR_INVALID_ARG;
+    if (time->deriv_mode != 0 && time->deriv_mode != 1) return JEFI_ERR_INVALID_ARG;
+    if (time->past_mode != 0) return JEFI_ERR_UNSUPPORTED;
+    if (device < 0) return JEFI_ERR_INVALID_ARG;
+
+    jefi_ctx* c = new (std::nothrow) jefi_ctx;
+    if (!c) return JEFI_ERR_OOM;
+    memset(c, 0, sizeof(*c));
+    jefi::Params& P = c->P;
+    P.Ns = 1; P.n_obs = 1;
+    for (int a = 0; a < 3; ++a) {
+        P.ns[a] = src->n[a]; P.so[a] = src->origin[a]; P.sh[a] = src->spacing[a];
+        P.Ns *= src->n[a];
+        if (obs->kind == 0) {
+            P.no[a] = obs->grid.n[a]; P.oo[a] = obs->grid.origin[a]; P.oh[a] = obs->grid.spacing[a];
+            P.n_obs *= obs->grid.n[a];
+        } else {
+            P.no[a] = 1; P.oo[a] = 0; P.oh[a] = 1;
+        }
+    }
+    if (obs->kind == 1) { P.n_obs = obs->npoints; P.no[0] = (int)(obs->npoints > 0x7fffffff ? 0x7fffffff : obs->npoints); }
+    P.obs_kind = obs->kind; P.obs_points = obs->points_dev;
+    P.T = time->nsteps; P.Tp = time->nsteps + 1;
+    P.dt = time->dt; P.c = time->c; P.deriv_mode = time->deriv_mode;
+    c->dtype = dtype; c->device = device; c->t0 = time->t0;
+    c->elem = dtype == JEFI_F32 ? sizeof(float) : sizeof(double);
+    if (P.Ns > (1LL << 31) - 64 || P.n_obs >= (1LL << 40)) { delete c; return JEFI_ERR_UNSUPPORTED; }
+
+    cudaError_t e = cudaSetDevice(device);
+    if (e != cudaSuccess) { cudaGetLastError(); delete c; return JEFI_ERR_CUDA; }
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, device);
+    if (e != cudaSuccess) { cudaGetLastError(); delete c; return JEFI_ERR_CUDA; }
+    c->sm_count = prop.multiProcessorCount;
+
+    // scratch: S chunks x 6 components x n_obs doubles; S*n_obs is kept near 16 waves of points
+    long long scratch_pts = P.n_obs;
+    const long long floor_pts = 64LL * 4096;
+    if (scratch_pts < floor_pts) scratch_pts = floor_pts;
+    c->scratch_elems = 6 * scratch_pts;
+
+    c->hist_bytes = (size_t)P.Ns * 2 * (size_t)P.Tp * 4 * c->elem;
+    jefi_status s;
+    if ((s = dev_alloc(c, &c->hist, c->hist_bytes, "cudaMalloc(packed history)")) != JEFI_OK ||
+        (s = dev_alloc(c, &c->scratch, (size_t)c->scratch_elems * sizeof(double), "cudaMalloc(scratch)")) != JEFI_OK ||
+        (s = dev_alloc(c, &c->stage_E, (size_t)P.n_obs * 3 * c->elem, "cudaMalloc(E staging)")) != JEFI_OK ||
+        (s = dev_alloc(c, &c->stage_B, (size_t)P.n_obs * 3 * c->elem, "cudaMalloc(B staging)")) != JEFI_OK) {
+        free_all(c); delete c; return s;
+    }
+    *out = c;
+    return JEFI_OK;
+}
+
+jefi_status jefi_upload_history(jefi_ctx* ctx, const void* rho_dev, const void* J_dev,
+                                jefi_stream stream)
+{
+    if (!ctx) return JEFI_ERR_INVALID_ARG;
+    ctx->err[0] = 0;
+    if (!rho_dev || !J_dev) { set_err(ctx, "null history pointer", cudaSuccess); return JEFI_ERR_INVALID_ARG; }
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e != cudaSuccess) return cuda_fail(ctx, "cudaSetDevice", e);
+    int n = jefi::launch_prepass(ctx->P, ctx->dtype, rho_dev, J_dev, ctx->hist, (cudaStream_t)stream);
+    if (n < 0) return cuda_fail(ctx, "pre-pass launch", cudaGetLastError());
+    ctx->launches += n;
+    ctx->has_history = true;
+    return JEFI_OK;
+}
+
+jefi_status jefi_upload_history_host(jefi_ctx* ctx, const void* rho_host, const void* J_host,
+                                     jefi_stream stream)
+{
+    if (!ctx) return JEFI_ERR_INVALID_ARG;
+    ctx->err[0] = 0;
+    if (!rho_host || !J_host) { set_err(ctx, "null history pointer", cudaSuccess); return JEFI_ERR_INVALID_ARG; }
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e != cudaSuccess) return cuda_fail(ctx, "cudaSetDevice", e);
+    const size_t rho_bytes = (size_t)ctx->P.T * (size_t)ctx->P.Ns * ctx->elem;
+    if (!ctx->raw_rho) {
+        jefi_status s;
+        if ((s = dev_alloc(ctx, &ctx->raw_rho, rho_bytes, "cudaMalloc(raw rho)")) != JEFI_OK) return s;
+        if ((s = dev_alloc(ctx, &ctx->raw_J, 3 * rho_bytes, "cudaMalloc(raw J)")) != JEFI_OK) return s;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((e = cudaMemcpyAsync(ctx->raw_rho, rho_host, rho_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+        return cuda_fail(ctx, "cudaMemcpyAsync(rho)", e);
+    if ((e = cudaMemcpyAsync(ctx->raw_J, J_host, 3 * rho_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+        return cuda_fail(ctx, "cudaMemcpyAsync(J)", e);
+    return jefi_upload_history(ctx, ctx->raw_rho, ctx->raw_J, stream);
+}
+
+jefi_status jefi_fields(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t obs_count,
+                        void* E_out_dev, void* B_out_dev, jefi_stream stream)
+{
+    jefi_status s = check_fields_args(ctx, step, obs_begin, obs_count, E_out_dev, B_out_dev);
+    if (s != JEFI_OK) return s;
+    return run_fields(ctx, step, obs_begin, obs_count, E_out_dev, B_out_dev, (cudaStream_t)stream);
+}
+
+jefi_status jefi_fields_at_time(jefi_ctx* ctx, double t, int64_t obs_begin, int64_t obs_count,
+                                void* E_out_dev, void* B_out_dev, jefi_stream stream)
+{
+    if (!ctx) return JEFI_ERR_INVALID_ARG;
+    ctx->err[0] = 0;
+    const double x = (t - ctx->t0) / ctx->P.dt;
+    const double n = floor(x + 0.5);
+    if (!isfinite(x) || fabs(x - n) > 1e-6 || n < 0.0 || n > (double)(ctx->P.T - 1)) {
+        set_err(ctx, "t is not on the stored step grid", cudaSuccess);
+        return JEFI_ERR_TIME_RANGE;
+    }
+    return jefi_fields(ctx, (int32_t)n, obs_begin, obs_count, E_out_dev, B_out_dev, stream);
+}
+
+jefi_status jefi_fields_host(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t obs_count,
+                             void* E_out_host, void* B_out_host, jefi_stream stream)
+{
+    jefi_status s = check_fields_args(ctx, step, obs_begin, obs_count, E_out_host, B_out_host);
+    if (s != JEFI_OK) return s;
+    if (obs_count == 0) return JEFI_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    s = run_fields(ctx, step, obs_begin, obs_count, ctx->stage_E, ctx->stage_B, st);
+    if (s != JEFI_OK) return s;
+    const size_t bytes = (size_t)obs_count * 3 * ctx->elem;
+    cudaError_t e;
+    if ((e = cudaMemcpyAsync(E_out_host, ctx->stage_E, bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+        return cuda_fail(ctx, "cudaMemcpyAsync(E)", e);
+    if ((e = cudaMemcpyAsync(B_out_host, ctx->stage_B, bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+        return cuda_fail(ctx, "cudaMemcpyAsync(B)", e);
+    return JEFI_OK;
+}
+
+jefi_status jefi_set_kernel(jefi_ctx* ctx, int32_t which)
+{
+    if (!ctx || which < 0 || which > 2) return JEFI_ERR_INVALID_ARG;
+    ctx->kernel_choice = which;
+    return JEFI_OK;
+}
+
+int64_t jefi_launch_count(const jefi_ctx* ctx) { return ctx ? ctx->launches : 0; }
+int64_t jefi_device_bytes(const jefi_ctx* ctx) { return ctx ? ctx->dev_bytes : 0; }
+
+jefi_status jefi_destroy(jefi_ctx* ctx)
+{
+    if (!ctx) return JEFI_ERR_INVALID_ARG;
+    jefi_status s = JEFI_OK;
+    if (cudaSetDevice(ctx->device) != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) {
+        cudaGetLastError();
+        s = JEFI_ERR_CUDA;
+    }
+    free_all(ctx);
+    delete ctx;
+    return s;
+}
+
+const char* jefi_status_string(jefi_status s)
+{
+    switch (s) {
+        case JEFI_OK: return "JEFI_OK";
+        case JEFI_ERR_INVALID_ARG: return "JEFI_ERR_INVALID_ARG";
+        case JEFI_ERR_CUDA: return "JEFI_ERR_CUDA";
+        case JEFI_ERR_OOM: return "JEFI_ERR_OOM";
+        case JEFI_ERR_NO_HISTORY: return "JEFI_ERR_NO_HISTORY";
+        case JEFI_ERR_TIME_RANGE: return "JEFI_ERR_TIME_RANGE";
+        case JEFI_ERR_UNSUPPORTED: return "JEFI_ERR_UNSUPPORTED";
+    }
+    return "JEFI_ERR_?";
+}
+
+const char* jefi_last_error(const jefi_ctx* ctx) { return ctx ? ctx->err : ""; }
+
+int jefi_flops_per_pair(void) { return 52; }
+
+jefi_status jefi_measure_alu_peak(int device, jefi_dtype dtype, double* tflops)
+{
+    if (!tflops || device < 0 || (dtype != JEFI_F32 && dtype != JEFI_F64)) return JEFI_ERR_INVALID_ARG;
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return JEFI_ERR_CUDA; }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaGetLastError(); return JEFI_ERR_CUDA; }
+    const double v = jefi::measure_alu_peak(dtype, prop.multiProcessorCount, 0);
+    if (v < 0) { cudaGetLastError(); return JEFI_ERR_CUDA; }
+    *tflops = v;
+    return JEFI_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,181 @@
+// pairwise_point.cu -- steps a2-a5 in the paper's own shape (Fig. 1): one
+// thread per observation point, a serial loop over source cells, history gathered straight
+// from global memory.  It is the general path (explicit point lists, any grid) and the
+// bring-up/cross-check kernel; the tiled kernel (pairwise_tiled.cu) is the fast path.
+// Also holds step a6, the deterministic reduce + scale + store epilogue both kernels share.
+//
+// Per pair (Eq. (4)-(6), in the pre-scaled variables of prepass.cu):
+//   d = r - r',  R^2 = d.d,  rinv = rsqrt(R^2) (0 if R^2 < rcut^2: screening)
+//   k = floor(R/(c dt) + 0.5),  p = max(n + 1 - k, 0)            (p = 0: the all-zero record)
+//   s = (rho*rinv + rho_dot')*rinv^2,   u = (J'*rinv + J_dot'')*rinv^2
+//   E += d*s - J_dot''*rinv,            B' += u x d               (B = c * B')
+#include "jefi_internal.h"
+
+namespace jefi {
+namespace {
+
+template <typename T> struct alignas(4 * sizeof(T)) Vec4 { T x, y, z, w; };
+
+template <typename T> __device__ __forceinline__ T rsqrt_t(T x);
+template <> __device__ __forceinline__ float  rsqrt_t<float>(float x)   { return rsqrtf(x); }
+template <> __device__ __forceinline__ double rsqrt_t<double>(double x) { return 1.0 / sqrt(x); }
+
+struct PointArgs {
+    int nsx, nsy, nsz;
+    int nox, noy;
+    double shx, shy, shz;       // source spacing
+    double ohx, ohy, ohz;       // obs spacing
+    double d0x, d0y, d0z;       // obs origin - source origin (host fp64)
+    double sox, soy, soz;       // source origin (for explicit point lists)
+    double rcut2, inv_cdt;
+    long long Ns, obs_begin, obs_count;
+    int Tp, n1;                 // n1 = step + 1
+    int obs_kind;
+    const void* points;
+    long long cells_per_chunk;
+};
+
+constexpr int kPointThreads = 128;
+
+template <typename T>
+__global__ void __launch_bounds__(kPointThreads)
+fields_point_kernel(const Vec4<T>* __restrict__ hist, double* __restrict__ partial, PointArgs a)
+{
+    const long long i = (long long)blockIdx.x * kPointThreads + threadIdx.x;
+    if (i >= a.obs_count) return;
+    const long long gi = a.obs_begin + i;
+
+    // observation position relative to the centre of source cell (0,0,0)
+    T ox, oy, oz;
+    if (a.obs_kind == 0) {
+        const int ix = (int)(gi % a.nox), iy = (int)((gi / a.nox) % a.noy);
+        const int iz = (int)(gi / ((long long)a.nox * a.noy));
+        ox = (T)(a.d0x + ix * a.ohx); oy = (T)(a.d0y + iy * a.ohy); oz = (T)(a.d0z + iz * a.ohz);
+    } else {
+        const T* p = (const T*)a.points + 3 * gi;
+        ox = (T)((double)p[0] - a.sox); oy = (T)((double)p[1] - a.soy); oz = (T)((double)p[2] - a.soz);
+    }
+    const T shx = (T)a.shx, shy = (T)a.shy, shz = (T)a.shz;
+    const T rcut2 = (T)a.rcut2, inv_cdt = (T)a.inv_cdt;
+
+    const long long cb = (long long)blockIdx.y * a.cells_per_chunk;
+    long long ce = cb + a.cells_per_chunk;
+    if (ce > a.Ns) ce = a.Ns;
+    int sx = (int)(cb % a.nsx), sy = (int)((cb / a.nsx) % a.nsy);
+    int sz = (int)(cb / ((long long)a.nsx * a.nsy));
+
+    double tot[6] = {0, 0, 0, 0, 0, 0};
+    long long j = cb;
+    while (j < ce) {
+        // one (part of a) source row: y, z fixed
+        const T dy = oy - (T)sy * shy, dz = oz - (T)sz * shz;
+        const T ryz = dy * dy + dz * dz;
+        long long row_end = j + (a.nsx - sx);
+        if (row_end > ce) row_end = ce;
+        T ex = 0, ey = 0, ez = 0, bx = 0, by = 0, bz = 0;
+        for (; j < row_end; ++j, ++sx) {
+            const T dx = ox - (T)sx * shx;
+            const T R2 = dx * dx + ryz;
+            T rinv = rsqrt_t<T>(R2);
+            if (R2 < rcut2) rinv = T(0);
+            const T R = R2 * rinv;
+            const int k = (int)floor(R * inv_cdt + T(0.5));
+            int p = a.n1 - k;
+            p = p < 0 ? 0 : p;
+            const Vec4<T> ha = hist[(j * 2 + 0) * a.Tp + p];
+            const Vec4<T> hb = hist[(j * 2 + 1) * a.Tp + p];
+            const T r2 = rinv * rinv;
+            const T s  = (ha.x * rinv + ha.y) * r2;
+            const T ux = (ha.z * rinv + hb.y) * r2;
+            const T uy = (ha.w * rinv + hb.z) * r2;
+            const T uz = (hb.x * rinv + hb.w) * r2;
+            ex += dx * s - hb.y * rinv;
+            ey += dy * s - hb.z * rinv;
+            ez += dz * s - hb.w * rinv;
+            bx += uy * dz - uz * dy;
+            by += uz * dx - ux * dz;
+            bz += ux * dy - uy * dx;
+        }
+        tot[0] += (double)ex; tot[1] += (double)ey; tot[2] += (double)ez;
+        tot[3] += (double)bx; tot[4] += (double)by; tot[5] += (double)bz;
+        sx = 0;
+        if (++sy == a.nsy) { sy = 0; ++sz; }
+    }
+    double* out = partial + (long long)blockIdx.y * 6 * a.obs_count + i;
+#pragma unroll
+    for (int c = 0; c < 6; ++c) out[(long long)c * a.obs_count] = tot[c];
+}
+
+// step a6: fixed-order sum over the S source chunks, scale, store as component planes
+template <typename T>
+__global__ void __launch_bounds__(256)
+reduce_scale_kernel(const double* __restrict__ partial, T* __restrict__ E, T* __restrict__ B,
+                    long long count, int S, double scaleE, double scaleB)
+{
+    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (i >= count) return;
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+        double acc = 0.0;
+        for (int s = 0; s < S; ++s) acc += partial[((long long)s * 6 + c) * count + i];
+        if (c < 3) E[(long long)c * count + i] = (T)(acc * scaleE);
+        else       B[(long long)(c - 3) * count + i] = (T)(acc * scaleB);
+    }
+}
+
+}  // namespace
+
+int launch_reduce_scale(const Params& P, jefi_dtype dt, const FieldsLaunch& L, int S)
+{
+    const double pi = 3.14159265358979323846;
+    const double dV = P.sh[0] * P.sh[1] * P.sh[2];
+    const double scaleE = dV / (4.0 * pi), scaleB = P.c * scaleE;
+    const unsigned grid = (unsigned)((L.obs_count + 255) / 256);
+    if (dt == JEFI_F32)
+        reduce_scale_kernel<float><<<grid, 256, 0, L.stream>>>(
+            (const double*)L.scratch, (float*)L.E_out, (float*)L.B_out, L.obs_count, S, scaleE, scaleB);
+    else
+        reduce_scale_kernel<double><<<grid, 256, 0, L.stream>>>(
+            (const double*)L.scratch, (double*)L.E_out, (double*)L.B_out, L.obs_count, S, scaleE, scaleB);
+    return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+}
+
+int launch_fields_point(const Params& P, jefi_dtype dt, const void* hist, const FieldsLaunch& L)
+{
+    PointArgs a;
+    a.nsx = P.ns[0]; a.nsy = P.ns[1]; a.nsz = P.ns[2];
+    a.nox = P.no[0]; a.noy = P.no[1];
+    a.shx = P.sh[0]; a.shy = P.sh[1]; a.shz = P.sh[2];
+    a.ohx = P.oh[0]; a.ohy = P.oh[1]; a.ohz = P.oh[2];
+    a.d0x = P.oo[0] - P.so[0]; a.d0y = P.oo[1] - P.so[1]; a.d0z = P.oo[2] - P.so[2];
+    a.sox = P.so[0]; a.soy = P.so[1]; a.soz = P.so[2];
+    double hmin = P.sh[0] < P.sh[1] ? P.sh[0] : P.sh[1];
+    hmin = hmin < P.sh[2] ? hmin : P.sh[2];
+    a.rcut2 = 0.25 * hmin * hmin;
+    a.inv_cdt = 1.0 / (P.c * P.dt);
+    a.Ns = P.Ns; a.obs_begin = L.obs_begin; a.obs_count = L.obs_count;
+    a.Tp = P.Tp; a.n1 = L.step + 1;
+    a.obs_kind = P.obs_kind; a.points = P.obs_points;
+
+    const long long blocks = (L.obs_count + kPointThreads - 1) / kPointThreads;
+    long long S = (4LL * L.sm_count + blocks - 1) / blocks;
+    if (S > 64) S = 64;
+    if (S > P.Ns / 64) S = P.Ns / 64;
+    if (S * 6 * L.obs_count > L.scratch_elems) S = L.scratch_elems / (6 * L.obs_count);
+    if (S < 1) S = 1;
+    a.cells_per_chunk = (P.Ns + S - 1) / S;
+    S = (P.Ns + a.cells_per_chunk - 1) / a.cells_per_chunk;
+
+    dim3 grid((unsigned)blocks, (unsigned)S);
+    if (dt == JEFI_F32)
+        fields_point_kernel<float><<<grid, kPointThreads, 0, L.stream>>>(
+            (const Vec4<float>*)hist, (double*)L.scratch, a);
+    else
+        fields_point_kernel<double><<<grid, kPointThreads, 0, L.stream>>>(
+            (const Vec4<double>*)hist, (double*)L.scratch, a);
+    if (cudaPeekAtLastError() != cudaSuccess) return -1;
+    if (launch_reduce_scale(P, dt, L, (int)S) < 0) return -1;
+    return 2;
+}
+
+}  // namespace jefi

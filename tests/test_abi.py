@@ -1,0 +1,106 @@
+"""The C-ABI library loads and exports every symbol include/jefi.h declares, and rejects bad
+arguments before touching the device (no compute calls: runs without a GPU)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(HERE)
+
+
+@pytest.fixture(scope="module")
+def jb():
+    from paper_2104_05426_b200 import build
+    build.build()
+    import paper_2104_05426_b200 as jb
+    return jb
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "jefi.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(jefi_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_header_symbols_are_exported(jb):
+    names = _declared_symbols()
+    assert len(names) >= 12
+    lib = C.CDLL(str(jb.LIB_PATH))
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in include/jefi.h but not exported"
+    assert set(names) == set(jb.EXPORTS)
+
+
+def test_binding_has_same_names(jb):
+    for n in _declared_symbols():
+        assert callable(getattr(jb, n)), n
+
+
+def test_flops_per_pair_and_status_strings(jb):
+    assert jb.jefi_flops_per_pair() == 52
+    assert jb.jefi_status_string(0) == "JEFI_OK"
+    assert jb.jefi_status_string(jb.JEFI_ERR_TIME_RANGE) == "JEFI_ERR_TIME_RANGE"
+    assert jb.jefi_last_error(None) == ""
+
+
+def _descs(jb, n=(4, 4, 4), h=(0.1, 0.1, 0.1), dt=0.05, c=1.0, T=8):
+    src = jb.make_grid(n, (0, 0, 0), h)
+    obs = jb.jefi_obs_desc()
+    obs.kind = 0
+    obs.grid = jb.make_grid(n, (0, 0, 0), h)
+    tm = jb.jefi_time_desc(0.0, dt, c, T, 0, 0)
+    return src, obs, tm
+
+
+@pytest.mark.parametrize("mutate,status", [
+    (lambda s, o, t: s.n.__setitem__(1, 0), 1),
+    (lambda s, o, t: s.spacing.__setitem__(2, -0.1), 1),
+    (lambda s, o, t: s.origin.__setitem__(0, float("nan")), 1),
+    (lambda s, o, t: setattr(o, "kind", 7), 1),
+    (lambda s, o, t: o.grid.n.__setitem__(0, -3), 1),
+    (lambda s, o, t: setattr(t, "dt", 0.0), 1),
+    (lambda s, o, t: setattr(t, "c", -1.0), 1),
+    (lambda s, o, t: setattr(t, "nsteps", 0), 1),
+    (lambda s, o, t: setattr(t, "deriv_mode", 2), 1),
+    (lambda s, o, t: setattr(t, "past_mode", 1), 6),
+])
+def test_create_rejects_bad_descriptors_before_any_cuda_call(jb, mutate, status):
+    src, obs, tm = _descs(jb)
+    mutate(src, obs, tm)
+    with pytest.raises(jb.JefiError) as e:
+        jb.jefi_create(src, obs, tm, jb.JEFI_F32, 0)
+    assert e.value.status == status
+
+
+def test_create_rejects_null_and_bad_dtype(jb):
+    src, obs, tm = _descs(jb)
+    for args in ((None, obs, tm, 0, 0), (src, None, tm, 0, 0), (src, obs, None, 0, 0), (src, obs, tm, 5, 0),
+                 (src, obs, tm, 0, -1)):
+        with pytest.raises(jb.JefiError) as e:
+            jb.jefi_create(*args)
+        assert e.value.status == jb.JEFI_ERR_INVALID_ARG
+
+
+def test_null_context_is_an_error_not_a_crash(jb):
+    lib = C.CDLL(str(jb.LIB_PATH))
+    lib.jefi_fields.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+    assert lib.jefi_fields(None, 0, 0, 0, None, None, None) == jb.JEFI_ERR_INVALID_ARG
+    lib.jefi_upload_history.argtypes = [C.c_void_p] * 4
+    assert lib.jefi_upload_history(None, None, None, None) == jb.JEFI_ERR_INVALID_ARG
+    lib.jefi_destroy.argtypes = [C.c_void_p]
+    assert lib.jefi_destroy(None) == jb.JEFI_ERR_INVALID_ARG
+    lib.jefi_measure_alu_peak.argtypes = [C.c_int, C.c_int, C.c_void_p]
+    assert lib.jefi_measure_alu_peak(0, 0, None) == jb.JEFI_ERR_INVALID_ARG
+
+
+def test_product_does_not_import_the_oracle():
+    """The product path must never route through oracle/ (or workloads' arithmetic-free data)."""
+    pkg = os.path.join(ROOT, "paper_2104_05426_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".h", ".cuh")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", text, flags=re.M), f
+                assert "jefi_oracle" not in text, f

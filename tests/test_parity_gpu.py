@@ -1,0 +1,255 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 CPU oracle on the same seeded
+inputs.  Bar (BASELINE.json north_star): relative L2 error per field component <= 1e-5 in fp64
+mode and <= 2e-4 in fp32 mode; a component that is identically zero in the oracle is measured
+against the whole field's norm (Q10).  All tests need a GPU."""
+import numpy as np
+import pytest
+
+import workloads as wl
+from conftest import rel_l2
+from gpu_util import gpu_fields, make_ctx, oracle_fields, tol_for, upload
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = [1, 0]        # 1 = per-point kernel, 0 = automatic (tiled where supported)
+
+
+@pytest.fixture(scope="module")
+def jb():
+    import paper_2104_05426_b200 as jb
+    return jb
+
+
+def check(w, E, B, Eo, Bo, tol=None, what=""):
+    tol = tol_for(w) if tol is None else tol
+    assert np.isfinite(E).all() and np.isfinite(B).all(), what
+    eE, eB = rel_l2(E, Eo, field_ref=Eo), rel_l2(B, Bo, field_ref=Bo)
+    assert max(eE) <= tol and max(eB) <= tol, f"{what}: rel-L2 E {eE} B {eB} tol {tol}"
+    return eE, eB
+
+
+def run_case(jb, w, idx, kernel, deriv_mode=0, steps=None, tol=None):
+    ctx = make_ctx(w, jb, deriv_mode)
+    try:
+        ctx.set_kernel(kernel)
+        upload(ctx, w)
+        for n in (w.steps if steps is None else steps):
+            E, B = gpu_fields(ctx, w, n)
+            Eo, Bo = oracle_fields(w, n, idx, deriv_mode)
+            sel = slice(None) if idx is None else idx
+            check(w, E[:, sel], B[:, sel], Eo, Bo, tol, f"{w.name} step {n} kernel {kernel}")
+        return E, B
+    finally:
+        ctx.close()
+
+
+# ------------------------------------------------------------------ config 1
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("deriv_mode", [0, 1])
+def test_config1_tiny_fp64_full(jb, kernel, deriv_mode):
+    run_case(jb, wl.config1_tiny(), None, kernel, deriv_mode)
+
+
+# ------------------------------------------------------------------ config 2
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config2a_coulomb(jb, kernel, dtype):
+    w = wl.config2a_coulomb(dtype)
+    E, B = run_case(jb, w, w.obs_subset(2048), kernel)
+    assert np.all(B == 0.0)                      # J = 0: every B term is an exact zero
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config2b_biot_savart(jb, kernel, dtype):
+    w = wl.config2b_wire(dtype)
+    E, B = run_case(jb, w, w.obs_subset(2048), kernel)
+    assert np.all(E == 0.0)
+    assert np.all(B[2] == 0.0)                   # J || z
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config2c_white_noise_history(jb, kernel, dtype):
+    """White in time: one wrong retarded index is an O(1) error in that term."""
+    w = wl.config2c_noise(dtype)
+    run_case(jb, w, w.obs_subset(2048), kernel)
+
+
+# ------------------------------------------------------------------ config 3 (the bench workload, full size)
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_config3_collision_full_size_sampled(jb, kernel):
+    w = wl.config3_collision()
+    assert w.T == 221 and w.N_s == 64 ** 3
+    run_case(jb, w, w.obs_subset(1024), kernel)
+
+
+# ------------------------------------------------------------------ config 4
+def test_config4_detached_plane_time_series(jb):
+    w = wl.config4_detached()
+    assert w.T == 622 and w.steps[0] == 494 and len(w.steps) == 128
+    idx = w.obs_subset(1536)
+    ctx = make_ctx(w, jb)
+    try:
+        upload(ctx, w)
+        checked = {w.steps[0], w.steps[-1], w.steps[37]}
+        for n in w.steps:
+            E, B = gpu_fields(ctx, w, n)
+            assert np.isfinite(E).all() and np.isfinite(B).all()
+            if n in checked:
+                Eo, Bo = oracle_fields(w, n, idx)
+                check(w, E[:, idx], B[:, idx], Eo, Bo, None, f"c4 step {n}")
+    finally:
+        ctx.close()
+
+
+# ------------------------------------------------------------------ config 5
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_config5_large_sampled(jb, dtype):
+    """100^3 x 100^3 with a history shorter than the longest delay (k_max = 343 > T-1 = 199):
+    the m < 0 rule (Q4) is live.  fp32: the whole grid; fp64: a 100x100x12 slab of it."""
+    w = wl.config5_large(dtype=dtype)
+    ctx = make_ctx(w, jb)
+    try:
+        upload(ctx, w)
+        n = w.steps[0]
+        if dtype == "f32":
+            begin, count = 0, w.N_o
+        else:
+            begin, count = 100 * 100 * 44, 100 * 100 * 12
+        E, B = gpu_fields(ctx, w, n, begin, count)
+        idx = w.obs_subset(400, seed_offset=1)
+        idx = idx[(idx >= begin) & (idx < begin + count)]
+        if dtype == "f64":
+            extra = begin + np.arange(0, count, 997)
+            idx = np.unique(np.concatenate([idx, extra]))[:320]
+        Eo, Bo = oracle_fields(w, n, idx)
+        check(w, E[:, idx - begin], B[:, idx - begin], Eo, Bo, None, f"c5 {dtype}")
+    finally:
+        ctx.close()
+
+
+# ------------------------------------------------------------------ ragged shapes, c != 1, sub-ranges, point lists
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_ragged_anisotropic_offset_grids_with_c(jb, kernel, dtype):
+    w = wl.random_history((13, 5, 7), 40, seed=77, dtype=dtype, spacing=(0.1, 0.15, 0.07),
+                          n_obs=(9, 11, 3), spacing_obs=(0.12, 0.05, 0.2), origin_obs=(-0.31, -0.22, 0.13),
+                          dt=0.02, c=1.7)
+    for mode in (0, 1):
+        run_case(jb, w, None, kernel, mode, steps=(39, 20, 3, 0))
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_overlapping_grid_hits_the_screening_rule(jb, kernel):
+    """obs == source centres (self cell at R = 0) plus points strictly inside / outside rcut."""
+    w = wl.random_history((6, 6, 6), 24, seed=5, dtype="f64", spacing=(0.1, 0.1, 0.1), dt=0.05)
+    run_case(jb, w, None, kernel)
+    w2 = wl.random_history((6, 6, 6), 24, seed=5, dtype="f64", spacing=(0.1, 0.1, 0.1), dt=0.05,
+                           origin_obs=(-0.25 + 0.03, -0.25, -0.25 + 0.02))     # R = 0.036 < 0.05
+    run_case(jb, w2, None, kernel)
+    w3 = wl.random_history((6, 6, 6), 24, seed=5, dtype="f64", spacing=(0.1, 0.1, 0.1), dt=0.05,
+                           origin_obs=(-0.25 + 0.04, -0.25 + 0.04, -0.25))     # R = 0.0566 > 0.05
+    run_case(jb, w3, None, kernel)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_single_stored_step_and_single_cell(jb, kernel):
+    w = wl.random_history((1, 1, 1), 1, seed=9, dtype="f64", n_obs=(3, 2, 2), spacing_obs=(0.01, 0.01, 0.01),
+                          origin_obs=(0.2, 0.0, 0.0), dt=10.0)
+    run_case(jb, w, None, kernel, steps=(0,))
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_obs_subranges_match_the_full_call(jb, kernel):
+    w = wl.random_history((8, 8, 4), 30, seed=11, dtype="f32", n_obs=(10, 7, 5), dt=0.04)
+    ctx = make_ctx(w, jb)
+    try:
+        ctx.set_kernel(kernel)
+        upload(ctx, w)
+        E, B = gpu_fields(ctx, w, 29)
+        for begin, count in ((0, 1), (3, 64), (117, 233), (349, 1), (0, 350)):
+            e, b = gpu_fields(ctx, w, 29, begin, count)
+            np.testing.assert_allclose(e, E[:, begin:begin + count], rtol=2e-5, atol=1e-6)
+            np.testing.assert_allclose(b, B[:, begin:begin + count], rtol=2e-5, atol=1e-6)
+        e, b = gpu_fields(ctx, w, 29, 5, 0)          # empty range is a no-op
+        assert e.shape == (3, 0)
+    finally:
+        ctx.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_explicit_point_list_matches_oracle(jb, dtype):
+    w = wl.random_history((7, 6, 5), 32, seed=13, dtype=dtype, dt=0.03)
+    u = wl.uniform01(4242, 0, 3 * 257).reshape(257, 3)
+    pts = (u - 0.5) * np.array([1.5, 1.2, 2.0])
+    pts = pts.astype(w.np_dtype).astype(np.float64)     # both sides see the same rounded points
+    ctx = make_ctx(w, jb, points=pts)
+    try:
+        upload(ctx, w)
+        E, B = gpu_fields(ctx, w, 31)
+        Eo, Bo = oracle_fields(w, 31, points=pts)
+        check(w, E, B, Eo, Bo, None, "point list")
+    finally:
+        ctx.close()
+
+
+def test_time_series_and_truncated_history(jb):
+    """Every step from 0: early steps have most of the light cone before the stored history."""
+    w = wl.random_history((6, 5, 4), 16, seed=21, dtype="f64", dt=0.05)
+    run_case(jb, w, None, 0, steps=tuple(range(16)))
+
+
+# ------------------------------------------------------------------ host-buffer entry points, errors
+def test_host_buffer_entry_points_match_device_ones(jb):
+    import torch
+    w = wl.random_history((8, 6, 5), 20, seed=31, dtype="f32", n_obs=(7, 5, 3), dt=0.05)
+    ctx = make_ctx(w, jb)
+    try:
+        rho_h = torch.from_numpy(w.rho).pin_memory()
+        J_h = torch.from_numpy(w.J).pin_memory()
+        ctx.upload_history_host(rho_h, J_h)
+        E_h = torch.empty((3, w.N_o), dtype=torch.float32).pin_memory()
+        B_h = torch.empty((3, w.N_o), dtype=torch.float32).pin_memory()
+        ctx.fields_host(19, E_h, B_h)
+        torch.cuda.synchronize()
+        E, B = gpu_fields(ctx, w, 19)
+        np.testing.assert_array_equal(E_h.numpy().astype(np.float64), E)
+        np.testing.assert_array_equal(B_h.numpy().astype(np.float64), B)
+        Eo, Bo = oracle_fields(w, 19)
+        check(w, E, B, Eo, Bo)
+    finally:
+        ctx.close()
+
+
+def test_error_codes_on_device(jb):
+    import torch
+    w = wl.random_history((4, 4, 4), 8, seed=1, dtype="f32")
+    ctx = make_ctx(w, jb)
+    try:
+        E = torch.empty((3, w.N_o), dtype=torch.float32, device="cuda")
+        B = torch.empty_like(E)
+        with pytest.raises(jb.JefiError) as e:
+            ctx.fields(7, E, B)
+        assert e.value.status == jb.JEFI_ERR_NO_HISTORY
+        upload(ctx, w)
+        for step in (-1, 8):
+            with pytest.raises(jb.JefiError) as e:
+                ctx.fields(step, E, B)
+            assert e.value.status == jb.JEFI_ERR_TIME_RANGE
+        with pytest.raises(jb.JefiError) as e:
+            ctx.fields(7, E, B, obs_begin=60, obs_count=5)
+        assert e.value.status == jb.JEFI_ERR_INVALID_ARG
+        with pytest.raises(jb.JefiError) as e:
+            jb.jefi_fields(ctx.ctx, 7, 0, w.N_o, None, B)
+        assert e.value.status == jb.JEFI_ERR_INVALID_ARG
+        with pytest.raises(jb.JefiError) as e:
+            jb.jefi_fields_at_time(ctx.ctx, 3.4 * w.dt, 0, w.N_o, E, B)
+        assert e.value.status == jb.JEFI_ERR_TIME_RANGE
+        jb.jefi_fields_at_time(ctx.ctx, 7 * w.dt, 0, w.N_o, E, B)
+        torch.cuda.synchronize()
+        E7, B7 = gpu_fields(ctx, w, 7)
+        np.testing.assert_array_equal(E.cpu().numpy().astype(np.float64), E7)
+        assert ctx.launches > 0
+    finally:
+        ctx.close()
