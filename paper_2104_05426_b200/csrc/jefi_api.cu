@@ -169,11 +169,13 @@ jefi_status jefi_create(const jefi_grid_desc* src, const jefi_obs_desc* obs,
     if (e != cudaSuccess) { cudaGetLastError(); delete c; return JEFI_ERR_CUDA; }
     c->sm_count = prop.multiProcessorCount;
 
-    // scratch: S chunks x 6 components x n_obs doubles; S*n_obs is kept near 16 waves of points
-    long long scratch_pts = P.n_obs;
-    const long long floor_pts = 64LL * 4096;
-    if (scratch_pts < floor_pts) scratch_pts = floor_pts;
-    c->scratch_elems = 6 * scratch_pts;
+    // scratch: partial sums [S chunks][6 components][points] in double.  Room for 16 chunks of the
+    // whole observation set (capped at 1 GiB, never below one chunk); the launchers choose S to fit.
+    long long pts = P.n_obs < 32768 ? 32768 : P.n_obs;
+    long long elems = 6 * 16 * pts;
+    if (elems > (1LL << 27)) elems = (1LL << 27);
+    if (elems < 6 * P.n_obs) elems = 6 * P.n_obs;
+    c->scratch_elems = elems;
 
     c->hist_bytes = (size_t)P.Ns * 2 * (size_t)P.Tp * 4 * c->elem;
     jefi_status s;
