@@ -14,7 +14,7 @@ struct jefi_ctx {
     double       t0;
     int          sm_count;
     size_t       elem;             // sizeof(float|double)
-    void*        hist;             // packed history, [N_s][2][Tp] vec4
+    void*        hist;             // packed history, [N_s][units][Tp], 16-byte units
     size_t       hist_bytes;
     void*        scratch;          // partial sums (double)
     long long    scratch_elems;

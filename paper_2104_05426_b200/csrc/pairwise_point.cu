@@ -14,7 +14,21 @@
 namespace jefi {
 namespace {
 
-template <typename T> struct alignas(4 * sizeof(T)) Vec4 { T x, y, z, w; };
+// packed history: [cell][unit][p] in 16-byte units (prepass.cu); a record is 8 values
+template <typename T> struct Rec { T v[8]; };
+__device__ __forceinline__ Rec<float> load_rec(const float* __restrict__ hist, long long j, int Tp, int p)
+{
+    const float4* h = reinterpret_cast<const float4*>(hist);
+    const float4 a = h[(j * 2 + 0) * Tp + p], b = h[(j * 2 + 1) * Tp + p];
+    return Rec<float>{{a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w}};
+}
+__device__ __forceinline__ Rec<double> load_rec(const double* __restrict__ hist, long long j, int Tp, int p)
+{
+    const double2* h = reinterpret_cast<const double2*>(hist);
+    const double2 a = h[(j * 4 + 0) * Tp + p], b = h[(j * 4 + 1) * Tp + p];
+    const double2 c = h[(j * 4 + 2) * Tp + p], d = h[(j * 4 + 3) * Tp + p];
+    return Rec<double>{{a.x, a.y, b.x, b.y, c.x, c.y, d.x, d.y}};
+}
 
 template <typename T> __device__ __forceinline__ T rsqrt_t(T x);
 template <> __device__ __forceinline__ float  rsqrt_t<float>(float x)   { return rsqrtf(x); }
@@ -39,7 +53,7 @@ constexpr int kPointThreads = 128;
 
 template <typename T>
 __global__ void __launch_bounds__(kPointThreads)
-fields_point_kernel(const Vec4<T>* __restrict__ hist, double* __restrict__ partial, PointArgs a)
+fields_point_kernel(const T* __restrict__ hist, double* __restrict__ partial, PointArgs a)
 {
     const long long i = (long long)blockIdx.x * kPointThreads + threadIdx.x;
     if (i >= a.obs_count) return;
@@ -82,16 +96,15 @@ fields_point_kernel(const Vec4<T>* __restrict__ hist, double* __restrict__ parti
             const int k = (int)floor(R * inv_cdt + T(0.5));
             int p = a.n1 - k;
             p = p < 0 ? 0 : p;
-            const Vec4<T> ha = hist[(j * 2 + 0) * a.Tp + p];
-            const Vec4<T> hb = hist[(j * 2 + 1) * a.Tp + p];
+            const Rec<T> h = load_rec(hist, j, a.Tp, p);      // rho, rho', Jx, Jy, Jz, Jx', Jy', Jz'
             const T r2 = rinv * rinv;
-            const T s  = (ha.x * rinv + ha.y) * r2;
-            const T ux = (ha.z * rinv + hb.y) * r2;
-            const T uy = (ha.w * rinv + hb.z) * r2;
-            const T uz = (hb.x * rinv + hb.w) * r2;
-            ex += dx * s - hb.y * rinv;
-            ey += dy * s - hb.z * rinv;
-            ez += dz * s - hb.w * rinv;
+            const T s  = (h.v[0] * rinv + h.v[1]) * r2;
+            const T ux = (h.v[2] * rinv + h.v[5]) * r2;
+            const T uy = (h.v[3] * rinv + h.v[6]) * r2;
+            const T uz = (h.v[4] * rinv + h.v[7]) * r2;
+            ex += dx * s - h.v[5] * rinv;
+            ey += dy * s - h.v[6] * rinv;
+            ez += dz * s - h.v[7] * rinv;
             bx += uy * dz - uz * dy;
             by += uz * dx - ux * dz;
             bz += ux * dy - uy * dx;
@@ -169,10 +182,10 @@ int launch_fields_point(const Params& P, jefi_dtype dt, const void* hist, const 
     dim3 grid((unsigned)blocks, (unsigned)S);
     if (dt == JEFI_F32)
         fields_point_kernel<float><<<grid, kPointThreads, 0, L.stream>>>(
-            (const Vec4<float>*)hist, (double*)L.scratch, a);
+            (const float*)hist, (double*)L.scratch, a);
     else
         fields_point_kernel<double><<<grid, kPointThreads, 0, L.stream>>>(
-            (const Vec4<double>*)hist, (double*)L.scratch, a);
+            (const double*)hist, (double*)L.scratch, a);
     if (cudaPeekAtLastError() != cudaSuccess) return -1;
     if (launch_reduce_scale(P, dt, L, (int)S) < 0) return -1;
     return 2;

@@ -8,8 +8,11 @@
 // In these variables Eq. (4)-(5) read  E = sum d (rho/R^3 + rho_dot'/R^2) - J_dot''/R  and
 // B = c * sum (J'/R^3 + J_dot''/R^2) x d, so the pairwise kernel never sees c.
 //
-// Output order is [cell][half][p], p = m + 1 (p = 0: all-zero record standing for every step
-// before the stored history).  A retarded-time window of one cell is then one contiguous run.
+// Output order is [cell][unit][p], p = m + 1 (p = 0: all-zero record standing for every step
+// before the stored history), in 16-byte units: fp32 has two units per record (the two float4
+// halves above), fp64 has four (double2: {rho, rho_dot'}, {Jx', Jy'}, {Jz', Jx_dot''},
+// {Jy_dot'', Jz_dot''}), so that consecutive steps of one unit are always 16 bytes apart and a
+// retarded-time window of one cell is one contiguous run per unit.
 // HBM-bound: 16 B read + 32 B written per record (fp32); the transpose from the cell-fastest
 // input to the time-fastest output goes through a padded shared-memory tile so that both the
 // global reads (lanes along cells) and the global writes (lanes along steps) are coalesced.
@@ -18,14 +21,16 @@
 namespace jefi {
 namespace {
 
-template <typename T> struct alignas(4 * sizeof(T)) Vec4 { T x, y, z, w; };
+template <typename T> struct Unit;                       // one 16-byte unit of a packed record
+template <> struct alignas(16) Unit<float>  { float v[4]; };
+template <> struct alignas(16) Unit<double> { double v[2]; };
 
 constexpr int kCells = 32;     // cells per tile
 constexpr int kThreads = 256;
 
 template <typename T, int TT>
 __global__ void __launch_bounds__(kThreads)
-prepass_kernel(const T* __restrict__ rho, const T* __restrict__ J, Vec4<T>* __restrict__ hist,
+prepass_kernel(const T* __restrict__ rho, const T* __restrict__ J, Unit<T>* __restrict__ hist,
                long long Ns, int Tsteps, int Tp, T inv_dt, T inv_c, int deriv_mode)
 {
     // raw[comp][row][cell(+1 pad)], row r <-> stored step m = p0 - 2 + r  (one halo row each side)
@@ -71,11 +76,16 @@ prepass_kernel(const T* __restrict__ rho, const T* __restrict__ J, Vec4<T>* __re
             f[comp] = fm; d[comp] = dd;
         }
         const T ic = inv_c, ic2 = inv_c * inv_c;
-        Vec4<T> a, b;
-        a.x = f[0];      a.y = d[0] * ic;  a.z = f[1] * ic;  a.w = f[2] * ic;
-        b.x = f[3] * ic; b.y = d[1] * ic2; b.z = d[2] * ic2; b.w = d[3] * ic2;
-        hist[(jj * 2 + 0) * Tp + p] = a;
-        hist[(jj * 2 + 1) * Tp + p] = b;
+        const T val[8] = {f[0], d[0] * ic, f[1] * ic, f[2] * ic, f[3] * ic, d[1] * ic2, d[2] * ic2, d[3] * ic2};
+        constexpr int U = sizeof(T) == 4 ? 2 : 4;                  // units per record
+        constexpr int VPU = 8 / U;                               // values per unit
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            Unit<T> q;
+#pragma unroll
+            for (int e = 0; e < VPU; ++e) q.v[e] = val[u * VPU + e];
+            hist[(jj * U + u) * Tp + p] = q;
+        }
     }
 }
 
@@ -89,13 +99,13 @@ int launch_prepass(const Params& P, jefi_dtype dt, const void* rho, const void* 
         constexpr int TT = 64;
         dim3 grid(gx, (unsigned)((P.Tp + TT - 1) / TT));
         prepass_kernel<float, TT><<<grid, kThreads, 0, stream>>>(
-            (const float*)rho, (const float*)J, (Vec4<float>*)hist, P.Ns, P.T, P.Tp,
+            (const float*)rho, (const float*)J, (Unit<float>*)hist, P.Ns, P.T, P.Tp,
             (float)(1.0 / P.dt), (float)(1.0 / P.c), P.deriv_mode);
     } else {
         constexpr int TT = 32;
         dim3 grid(gx, (unsigned)((P.Tp + TT - 1) / TT));
         prepass_kernel<double, TT><<<grid, kThreads, 0, stream>>>(
-            (const double*)rho, (const double*)J, (Vec4<double>*)hist, P.Ns, P.T, P.Tp,
+            (const double*)rho, (const double*)J, (Unit<double>*)hist, P.Ns, P.T, P.Tp,
             1.0 / P.dt, 1.0 / P.c, P.deriv_mode);
     }
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
