@@ -137,6 +137,16 @@ const char* jefi_last_error(const jefi_ctx* ctx);
  * the flop count of the oracle's loop body. */
 int         jefi_flops_per_pair(void);
 
+/* Host-only helper for one-process-per-GPU runs (the paper's one source-observation pair per
+ * GPU card): the contiguous slice [*begin, *begin + *count) of the observation
+ * set that rank `rank` of `world` evaluates when one history is replicated and the observation
+ * points are partitioned.  Slices are disjoint, cover the set in rank order, and are made of
+ * whole z-layers of a regular grid when there are at least `world` layers (else whole x-rows,
+ * else single points); sizes differ by at most one such granule.  Touches no device.
+ * JEFI_ERR_INVALID_ARG on null pointers, world <= 0 or rank outside [0, world). */
+jefi_status jefi_shard_obs(const jefi_obs_desc* obs, int32_t rank, int32_t world,
+                           int64_t* begin, int64_t* count);
+
 /* Register-only FFMA (dtype F32) or DFMA (dtype F64) chain on `device`: returns the measured
  * TFLOP/s in *tflops (synchronous; used by the bench to state the ALU peak it divides by). */
 jefi_status jefi_measure_alu_peak(int device, jefi_dtype dtype, double* tflops);

@@ -3,7 +3,7 @@
 Every step of the path (pre-pass, pairwise kernel, reduce/scale epilogue) runs in the CUDA
 kernels behind the C ABI; PyTorch is used by callers only to allocate device memory and to
 supply streams.  There is no CPU fallback: if the shared library has not been built
-(``python -m paper_2104_05426_b200.build``) importing this package raises.
+(``python paper_2104_05426_b200/build.py``) importing this package raises.
 The functions carry the names of the C entry points; ``Jefi`` is a small owner object around
 them for tests and the bench.
 """
@@ -23,7 +23,7 @@ EXPORTS = (
     "jefi_create", "jefi_upload_history", "jefi_upload_history_host", "jefi_fields",
     "jefi_fields_at_time", "jefi_fields_host", "jefi_set_kernel", "jefi_launch_count",
     "jefi_device_bytes", "jefi_destroy", "jefi_status_string", "jefi_last_error",
-    "jefi_flops_per_pair", "jefi_measure_alu_peak",
+    "jefi_flops_per_pair", "jefi_measure_alu_peak", "jefi_shard_obs",
 )
 
 
@@ -50,7 +50,7 @@ class JefiError(RuntimeError):
 
 if not LIB_PATH.exists():
     raise ImportError(
-        f"{LIB_PATH} is missing: build it with `python -m paper_2104_05426_b200.build` "
+        f"{LIB_PATH} is missing: build it with `python paper_2104_05426_b200/build.py` "
         "(nvcc, sm_100a).  There is no fallback path.")
 
 _lib = C.CDLL(str(LIB_PATH))
@@ -74,6 +74,8 @@ _lib.jefi_last_error.argtypes = [_P]
 _lib.jefi_last_error.restype = C.c_char_p
 _lib.jefi_flops_per_pair.argtypes = []
 _lib.jefi_measure_alu_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
+_lib.jefi_shard_obs.argtypes = [C.POINTER(jefi_obs_desc), C.c_int32, C.c_int32, C.POINTER(C.c_int64),
+                                C.POINTER(C.c_int64)]
 for _n in EXPORTS:
     if _n not in ("jefi_launch_count", "jefi_device_bytes", "jefi_status_string", "jefi_last_error"):
         getattr(_lib, _n).restype = C.c_int
@@ -182,6 +184,23 @@ def jefi_measure_alu_peak(device: int, dtype: int) -> float:
     if st != JEFI_OK:
         raise JefiError(st, "jefi_measure_alu_peak")
     return v.value
+
+
+def jefi_shard_obs(obs: jefi_obs_desc, rank: int, world: int):
+    """(begin, count) of the observation slice rank `rank` of `world` evaluates."""
+    b, n = C.c_int64(), C.c_int64()
+    st = _lib.jefi_shard_obs(C.byref(obs) if obs is not None else None, int(rank), int(world), C.byref(b),
+                             C.byref(n))
+    if st != JEFI_OK:
+        raise JefiError(st, "jefi_shard_obs")
+    return b.value, n.value
+
+
+def make_obs_grid(n, origin, spacing) -> jefi_obs_desc:
+    obs = jefi_obs_desc()
+    obs.kind = 0
+    obs.grid = make_grid(n, origin, spacing)
+    return obs
 
 
 # ------------------------------------------------------------------ owner object

@@ -1,6 +1,6 @@
 """Builds libjefi.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-    python -m paper_2104_05426_b200.build [--force] [--verbose]
+    python paper_2104_05426_b200/build.py [--force] [--verbose]
 
 Each csrc/*.cu is compiled to an object (in parallel) and linked into
 paper_2104_05426_b200/libjefi.so.  Nothing outside the package is touched.

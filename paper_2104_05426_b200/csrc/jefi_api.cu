@@ -307,6 +307,28 @@ const char* jefi_last_error(const jefi_ctx* ctx) { return ctx ? ctx->err : ""; }
 
 int jefi_flops_per_pair(void) { return 52; }
 
+jefi_status jefi_shard_obs(const jefi_obs_desc* obs, int32_t rank, int32_t world,
+                           int64_t* begin, int64_t* count)
+{
+    if (!obs || !begin || !count || world <= 0 || rank < 0 || rank >= world) return JEFI_ERR_INVALID_ARG;
+    if (obs->kind != 0 && obs->kind != 1) return JEFI_ERR_INVALID_ARG;
+    int64_t total, granule = 1;
+    if (obs->kind == 0) {
+        if (!grid_ok(obs->grid)) return JEFI_ERR_INVALID_ARG;
+        const int64_t nx = obs->grid.n[0], ny = obs->grid.n[1], nz = obs->grid.n[2];
+        total = nx * ny * nz;
+        if (nz >= world) granule = nx * ny;
+        else if (ny * nz >= world) granule = nx;
+    } else {
+        if (obs->npoints < 0) return JEFI_ERR_INVALID_ARG;
+        total = obs->npoints;
+    }
+    const int64_t units = total / granule, base = units / world, rem = units % world;
+    *begin = (rank * base + (rank < rem ? rank : rem)) * granule;
+    *count = (base + (rank < rem ? 1 : 0)) * granule;
+    return JEFI_OK;
+}
+
 jefi_status jefi_measure_alu_peak(int device, jefi_dtype dtype, double* tflops)
 {
     if (!tflops || device < 0 || (dtype != JEFI_F32 && dtype != JEFI_F64)) return JEFI_ERR_INVALID_ARG;

@@ -12,8 +12,8 @@ ROOT = os.path.dirname(HERE)
 
 @pytest.fixture(scope="module")
 def jb():
-    from paper_2104_05426_b200 import build
-    build.build()
+    import __graft_entry__
+    __graft_entry__.build()          # loads build.py by path (the package raises without its .so)
     import paper_2104_05426_b200 as jb
     return jb
 

@@ -1,0 +1,102 @@
+"""N > 1 host logic on CPU: world_size 2 over the gloo backend (no GPU).
+
+The method has no exchange step: ranks either run one S-O pair each
+(bench.py --gpus N) or partition one observation set with jefi_shard_obs.  Covered here:
+the partition rule (disjoint, ordered, complete, whole z-layers), that evaluating the slices
+separately and concatenating them in rank order equals the unsharded evaluation (the oracle
+stands in for the kernels: this test is about the slicing, not the arithmetic), and the
+max-over-ranks reduction bench.py uses for its timing."""
+import os
+import socket
+
+import numpy as np
+import pytest
+
+import workloads as wl
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, out_dir):
+    import torch
+    import torch.distributed as dist
+    import oracle
+    import paper_2104_05426_b200 as jb
+    import bench
+
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        w = wl.random_history((5, 4, 3), 12, seed=3, dtype="f64", n_obs=(4, 3, 5), dt=0.05)
+        obs = jb.make_obs_grid(w.n_obs, w.origin_obs, w.spacing_obs)
+        begin, count = jb.jefi_shard_obs(obs, rank, world)
+        idx = np.arange(begin, begin + count)
+        E, B = oracle.fields(w.n_src, w.origin_src, w.spacing_src, w.rho, w.J, dt=w.dt, c=w.c, step=11,
+                             obs_xyz=w.obs_points(idx), nthreads=1)
+        # gather the slices (sizes differ by a z-layer: pad to the largest)
+        sizes = [torch.zeros(1, dtype=torch.int64) for _ in range(world)]
+        dist.all_gather(sizes, torch.tensor([count], dtype=torch.int64))
+        cap = int(max(int(s) for s in sizes))
+        mine = torch.zeros((6, cap), dtype=torch.float64)
+        mine[:3, :count] = torch.from_numpy(E)
+        mine[3:, :count] = torch.from_numpy(B)
+        parts = [torch.zeros_like(mine) for _ in range(world)]
+        dist.all_gather(parts, mine)
+        full = torch.cat([p[:, :int(s)] for p, s in zip(parts, sizes)], dim=1).numpy()
+        # the timing reduction of bench.py: every rank ends with the slowest rank's numbers
+        red = bench.max_over_ranks([10.0 + rank, 5.0 - rank], device="cpu")
+        if rank == 0:
+            np.save(os.path.join(out_dir, "full.npy"), full)
+            np.save(os.path.join(out_dir, "red.npy"), np.array(red))
+            np.save(os.path.join(out_dir, "sizes.npy"), np.array([int(s) for s in sizes]))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_ranks_partition_the_observation_set(tmp_path):
+    import torch.multiprocessing as mp
+    import oracle
+    import __graft_entry__
+    __graft_entry__.build()
+    world = 2
+    mp.spawn(_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    full = np.load(tmp_path / "full.npy")
+    w = wl.random_history((5, 4, 3), 12, seed=3, dtype="f64", n_obs=(4, 3, 5), dt=0.05)
+    E, B = oracle.fields(w.n_src, w.origin_src, w.spacing_src, w.rho, w.J, dt=w.dt, c=w.c, step=11,
+                         obs_xyz=w.obs_points(), nthreads=1)
+    np.testing.assert_array_equal(full[:3], E)
+    np.testing.assert_array_equal(full[3:], B)
+    assert list(np.load(tmp_path / "sizes.npy")) == [36, 24]        # 3 + 2 z-layers of 4 x 3
+    assert list(np.load(tmp_path / "red.npy")) == [11.0, 5.0]
+
+
+@pytest.mark.parametrize("n,world", [((64, 64, 64), 8), ((256, 256, 1), 8), ((100, 100, 100), 3),
+                                     ((3, 2, 1), 4), ((5, 1, 1), 8), ((7, 9, 2), 5)])
+def test_shard_rule_is_a_partition(n, world):
+    import __graft_entry__
+    __graft_entry__.build()
+    import paper_2104_05426_b200 as jb
+    obs = jb.make_obs_grid(n, (0, 0, 0), (1, 1, 1))
+    total = n[0] * n[1] * n[2]
+    pos, counts = 0, []
+    for r in range(world):
+        b, c = jb.jefi_shard_obs(obs, r, world)
+        assert b == pos and c >= 0
+        pos += c
+        counts.append(c)
+    assert pos == total
+    granule = n[0] * n[1] if n[2] >= world else (n[0] if n[1] * n[2] >= world else 1)
+    assert all(c % granule == 0 for c in counts)
+    assert max(counts) - min(counts) <= granule
+    pts = jb.jefi_obs_desc()
+    pts.kind, pts.npoints = 1, 1001
+    got = [jb.jefi_shard_obs(pts, r, world) for r in range(world)]
+    assert sum(c for _, c in got) == 1001 and got[0][0] == 0
+    for bad in ((-1, world), (world, world), (0, 0)):
+        with pytest.raises(jb.JefiError):
+            jb.jefi_shard_obs(obs, *bad)
