@@ -94,7 +94,12 @@ jefi_status jefi_upload_history(jefi_ctx* ctx, const void* rho_dev, const void* 
                                 jefi_stream stream);
 
 /* Same, from HOST buffers (pinned for a truly asynchronous copy): copies them into a raw
- * device staging area owned by the context (allocated on first use) and runs the pre-pass. */
+ * device staging area owned by the context (allocated on first use) and runs the pre-pass on
+ * `stream`.  The host-to-device copy itself is enqueued on a stream owned by the context and
+ * `stream` waits for it, so in a stepping loop the copy of the next history overlaps the
+ * pairwise kernel of the current step.  Consequence: the host buffers must hold their data when
+ * this call is made (the copy is not ordered after earlier work on `stream`) and must stay
+ * untouched until `stream` has passed this call. */
 jefi_status jefi_upload_history_host(jefi_ctx* ctx, const void* rho_host, const void* J_host,
                                      jefi_stream stream);
 

@@ -22,6 +22,10 @@ struct jefi_ctx {
     void*        stage_B;
     void*        raw_rho;          // device staging for jefi_upload_history_host (lazy)
     void*        raw_J;
+    cudaStream_t copy_stream;      // H2D of the raw history runs here, beside the caller's stream
+    cudaEvent_t  ev_copied;        // copy_stream: raw staging filled
+    cudaEvent_t  ev_raw_free;      // caller's stream: the pre-pass has consumed the raw staging
+    bool         raw_in_use;
     bool         has_history;
     int          kernel_choice;
     long long    launches;
@@ -67,6 +71,9 @@ void free_all(jefi_ctx* c)
 {
     cudaFree(c->hist); cudaFree(c->scratch); cudaFree(c->stage_E); cudaFree(c->stage_B);
     cudaFree(c->raw_rho); cudaFree(c->raw_J);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->ev_copied) cudaEventDestroy(c->ev_copied);
+    if (c->ev_raw_free) cudaEventDestroy(c->ev_raw_free);
 }
 
 jefi_status check_fields_args(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t obs_count,
@@ -218,12 +225,32 @@ jefi_status jefi_upload_history_host(jefi_ctx* ctx, const void* rho_host, const 
         if ((s = dev_alloc(ctx, &ctx->raw_rho, rho_bytes, "cudaMalloc(raw rho)")) != JEFI_OK) return s;
         if ((s = dev_alloc(ctx, &ctx->raw_J, 3 * rho_bytes, "cudaMalloc(raw J)")) != JEFI_OK) return s;
     }
-    cudaStream_t st = (cudaStream_t)stream;
-    if ((e = cudaMemcpyAsync(ctx->raw_rho, rho_host, rho_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+    // The copy goes on the context's own stream so that, in a stepping loop, the H2D of the next
+    // history overlaps the pairwise kernel of the current step still running on `stream`:
+    //   copy_stream: wait(raw staging free) -> H2D rho, J -> record(copied)
+    //   stream:      wait(copied) -> pre-pass -> record(raw staging free)
+    if (!ctx->copy_stream) {
+        if ((e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking)) != cudaSuccess ||
+            (e = cudaEventCreateWithFlags(&ctx->ev_copied, cudaEventDisableTiming)) != cudaSuccess ||
+            (e = cudaEventCreateWithFlags(&ctx->ev_raw_free, cudaEventDisableTiming)) != cudaSuccess)
+            return cuda_fail(ctx, "copy stream/event creation", e);
+    }
+    cudaStream_t st = (cudaStream_t)stream, cs = ctx->copy_stream;
+    if (ctx->raw_in_use && (e = cudaStreamWaitEvent(cs, ctx->ev_raw_free, 0)) != cudaSuccess)
+        return cuda_fail(ctx, "cudaStreamWaitEvent(raw free)", e);
+    if ((e = cudaMemcpyAsync(ctx->raw_rho, rho_host, rho_bytes, cudaMemcpyHostToDevice, cs)) != cudaSuccess)
         return cuda_fail(ctx, "cudaMemcpyAsync(rho)", e);
-    if ((e = cudaMemcpyAsync(ctx->raw_J, J_host, 3 * rho_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+    if ((e = cudaMemcpyAsync(ctx->raw_J, J_host, 3 * rho_bytes, cudaMemcpyHostToDevice, cs)) != cudaSuccess)
         return cuda_fail(ctx, "cudaMemcpyAsync(J)", e);
-    return jefi_upload_history(ctx, ctx->raw_rho, ctx->raw_J, stream);
+    if ((e = cudaEventRecord(ctx->ev_copied, cs)) != cudaSuccess ||
+        (e = cudaStreamWaitEvent(st, ctx->ev_copied, 0)) != cudaSuccess)
+        return cuda_fail(ctx, "cudaEventRecord/WaitEvent(copied)", e);
+    jefi_status s = jefi_upload_history(ctx, ctx->raw_rho, ctx->raw_J, stream);
+    if (s != JEFI_OK) return s;
+    if ((e = cudaEventRecord(ctx->ev_raw_free, st)) != cudaSuccess)
+        return cuda_fail(ctx, "cudaEventRecord(raw free)", e);
+    ctx->raw_in_use = true;
+    return JEFI_OK;
 }
 
 jefi_status jefi_fields(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t obs_count,
