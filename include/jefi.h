@@ -103,6 +103,26 @@ jefi_status jefi_upload_history(jefi_ctx* ctx, const void* rho_dev, const void* 
 jefi_status jefi_upload_history_host(jefi_ctx* ctx, const void* rho_host, const void* J_host,
                                      jefi_stream stream);
 
+/* Sliding window.  The paper keeps as many snapshots as the longest light-travel time needs,
+ * lts = ceil(d_m/dt), resident on the GPU between calls, while the
+ * source solver keeps producing new ones.  jefi_append_step drops the oldest stored
+ * step and appends rho_new_dev[N_s], J_new_dev[3][N_s] as the new newest one: afterwards stored
+ * step m holds what step m+1 held, t0 has advanced by dt, and nsteps is unchanged (evaluate the
+ * new snapshot with step = nsteps-1).  Time derivatives follow deriv_mode: the new step gets
+ * (f_new - f_prev)/dt; in centred mode the previous newest step is re-differenced to
+ * (f_new - f_prev2)/(2 dt) now that it has a successor, and every other record -- the new oldest
+ * one included -- keeps the value it had.  The packed history therefore equals, record for
+ * record and bit for bit, the last nsteps records of a pre-pass over the (nsteps+1)-step raw
+ * history [old steps..., new step].  Needs a prior jefi_upload_history (JEFI_ERR_NO_HISTORY).
+ * One kernel on `stream`: an in-place shift of the packed history (read + write of it once). */
+jefi_status jefi_append_step(jefi_ctx* ctx, const void* rho_new_dev, const void* J_new_dev,
+                             jefi_stream stream);
+
+/* Same from HOST buffers rho_new_host[N_s], J_new_host[3][N_s] (copied on `stream` into a
+ * staging area owned by the context, allocated on first use). */
+jefi_status jefi_append_step_host(jefi_ctx* ctx, const void* rho_new_host, const void* J_new_host,
+                                  jefi_stream stream);
+
 /* Steps a2-a6: E and B at evaluation step `step` (t = t0 + step*dt) for the observation
  * points obs_begin .. obs_begin+obs_count-1 (linear indices into the observation set).
  * E_out_dev / B_out_dev are [3][obs_count] component planes of the context dtype, owned by

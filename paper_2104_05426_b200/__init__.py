@@ -24,6 +24,7 @@ EXPORTS = (
     "jefi_fields_at_time", "jefi_fields_host", "jefi_set_kernel", "jefi_launch_count",
     "jefi_device_bytes", "jefi_destroy", "jefi_status_string", "jefi_last_error",
     "jefi_flops_per_pair", "jefi_measure_alu_peak", "jefi_shard_obs",
+    "jefi_append_step", "jefi_append_step_host",
 )
 
 
@@ -59,6 +60,8 @@ _lib.jefi_create.argtypes = [C.POINTER(jefi_grid_desc), C.POINTER(jefi_obs_desc)
                              C.POINTER(jefi_time_desc), C.c_int, C.c_int, C.POINTER(_P)]
 _lib.jefi_upload_history.argtypes = [_P, _P, _P, _P]
 _lib.jefi_upload_history_host.argtypes = [_P, _P, _P, _P]
+_lib.jefi_append_step.argtypes = [_P, _P, _P, _P]
+_lib.jefi_append_step_host.argtypes = [_P, _P, _P, _P]
 _lib.jefi_fields.argtypes = [_P, C.c_int32, C.c_int64, C.c_int64, _P, _P, _P]
 _lib.jefi_fields_at_time.argtypes = [_P, C.c_double, C.c_int64, C.c_int64, _P, _P, _P]
 _lib.jefi_fields_host.argtypes = [_P, C.c_int32, C.c_int64, C.c_int64, _P, _P, _P]
@@ -143,6 +146,15 @@ def jefi_upload_history(ctx, rho_dev, J_dev, stream=None):
 def jefi_upload_history_host(ctx, rho_host, J_host, stream=None):
     _check(_lib.jefi_upload_history_host(ctx, _ptr(rho_host), _ptr(J_host), _stream(stream)), ctx,
            "jefi_upload_history_host")
+
+
+def jefi_append_step(ctx, rho_new_dev, J_new_dev, stream=None):
+    _check(_lib.jefi_append_step(ctx, _ptr(rho_new_dev), _ptr(J_new_dev), _stream(stream)), ctx, "jefi_append_step")
+
+
+def jefi_append_step_host(ctx, rho_new_host, J_new_host, stream=None):
+    _check(_lib.jefi_append_step_host(ctx, _ptr(rho_new_host), _ptr(J_new_host), _stream(stream)), ctx,
+           "jefi_append_step_host")
 
 
 def jefi_fields(ctx, step, obs_begin, obs_count, E_out_dev, B_out_dev, stream=None):
@@ -233,6 +245,12 @@ class Jefi:
 
     def upload_history_host(self, rho_host, J_host, stream=None):
         jefi_upload_history_host(self.ctx, rho_host, J_host, stream)
+
+    def append_step(self, rho_new_dev, J_new_dev, stream=None):
+        jefi_append_step(self.ctx, rho_new_dev, J_new_dev, stream)
+
+    def append_step_host(self, rho_new_host, J_new_host, stream=None):
+        jefi_append_step_host(self.ctx, rho_new_host, J_new_host, stream)
 
     def fields(self, step, E_out_dev, B_out_dev, obs_begin=0, obs_count=None, stream=None):
         n = self.n_points - obs_begin if obs_count is None else obs_count

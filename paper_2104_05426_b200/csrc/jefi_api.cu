@@ -20,6 +20,8 @@ struct jefi_ctx {
     long long    scratch_elems;
     void*        stage_E;          // device staging for jefi_fields_host, [3][N_o]
     void*        stage_B;
+    void*        last;             // raw values of the two newest stored steps, [2][4][N_s]
+    void*        new_stage;        // device staging for jefi_append_step_host, [4][N_s] (lazy)
     void*        raw_rho;          // device staging for jefi_upload_history_host (lazy)
     void*        raw_J;
     cudaStream_t copy_stream;      // H2D of the raw history runs here, beside the caller's stream
@@ -70,7 +72,7 @@ jefi_status dev_alloc(jefi_ctx* c, void** p, size_t bytes, const char* what)
 void free_all(jefi_ctx* c)
 {
     cudaFree(c->hist); cudaFree(c->scratch); cudaFree(c->stage_E); cudaFree(c->stage_B);
-    cudaFree(c->raw_rho); cudaFree(c->raw_J);
+    cudaFree(c->raw_rho); cudaFree(c->raw_J); cudaFree(c->last); cudaFree(c->new_stage);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->ev_copied) cudaEventDestroy(c->ev_copied);
     if (c->ev_raw_free) cudaEventDestroy(c->ev_raw_free);
@@ -188,6 +190,7 @@ jefi_status jefi_create(const jefi_grid_desc* src, const jefi_obs_desc* obs,
     jefi_status s;
     if ((s = dev_alloc(c, &c->hist, c->hist_bytes, "cudaMalloc(packed history)")) != JEFI_OK ||
         (s = dev_alloc(c, &c->scratch, (size_t)c->scratch_elems * sizeof(double), "cudaMalloc(scratch)")) != JEFI_OK ||
+        (s = dev_alloc(c, &c->last, (size_t)P.Ns * 8 * c->elem, "cudaMalloc(newest raw steps)")) != JEFI_OK ||
         (s = dev_alloc(c, &c->stage_E, (size_t)P.n_obs * 3 * c->elem, "cudaMalloc(E staging)")) != JEFI_OK ||
         (s = dev_alloc(c, &c->stage_B, (size_t)P.n_obs * 3 * c->elem, "cudaMalloc(B staging)")) != JEFI_OK) {
         free_all(c); delete c; return s;
@@ -207,8 +210,71 @@ jefi_status jefi_upload_history(jefi_ctx* ctx, const void* rho_dev, const void* 
     int n = jefi::launch_prepass(ctx->P, ctx->dtype, rho_dev, J_dev, ctx->hist, (cudaStream_t)stream);
     if (n < 0) return cuda_fail(ctx, "pre-pass launch", cudaGetLastError());
     ctx->launches += n;
+    // keep the raw values of the two newest steps for jefi_append_step (copies, no arithmetic)
+    {
+        const size_t plane = (size_t)ctx->P.Ns * ctx->elem;
+        const int T = ctx->P.T;
+        char* last = (char*)ctx->last;
+        const char* r = (const char*)rho_dev;
+        const char* Jp = (const char*)J_dev;
+        cudaStream_t st = (cudaStream_t)stream;
+        for (int s = 0; s < 2 && e == cudaSuccess; ++s) {
+            const int m = T - 2 + s;
+            if (m < 0) { e = cudaMemsetAsync(last + (size_t)s * 4 * plane, 0, 4 * plane, st); continue; }
+            e = cudaMemcpyAsync(last + (size_t)s * 4 * plane, r + (size_t)m * plane, plane,
+                                cudaMemcpyDeviceToDevice, st);
+            if (e == cudaSuccess)
+                e = cudaMemcpyAsync(last + ((size_t)s * 4 + 1) * plane, Jp + (size_t)m * 3 * plane, 3 * plane,
+                                    cudaMemcpyDeviceToDevice, st);
+        }
+        if (e != cudaSuccess) return cuda_fail(ctx, "copy of the newest raw steps", e);
+    }
     ctx->has_history = true;
     return JEFI_OK;
+}
+
+jefi_status jefi_append_step(jefi_ctx* ctx, const void* rho_new_dev, const void* J_new_dev, jefi_stream stream)
+{
+    if (!ctx) return JEFI_ERR_INVALID_ARG;
+    ctx->err[0] = 0;
+    if (!rho_new_dev || !J_new_dev) { set_err(ctx, "null step pointer", cudaSuccess); return JEFI_ERR_INVALID_ARG; }
+    if (!ctx->has_history) {
+        set_err(ctx, "jefi_append_step before jefi_upload_history", cudaSuccess);
+        return JEFI_ERR_NO_HISTORY;
+    }
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e != cudaSuccess) return cuda_fail(ctx, "cudaSetDevice", e);
+    int n = jefi::launch_append(ctx->P, ctx->dtype, rho_new_dev, J_new_dev, ctx->last, ctx->hist,
+                                (cudaStream_t)stream);
+    if (n < 0) return cuda_fail(ctx, "append launch", cudaGetLastError());
+    ctx->launches += n;
+    ctx->t0 += ctx->P.dt;
+    return JEFI_OK;
+}
+
+jefi_status jefi_append_step_host(jefi_ctx* ctx, const void* rho_new_host, const void* J_new_host,
+                                  jefi_stream stream)
+{
+    if (!ctx) return JEFI_ERR_INVALID_ARG;
+    ctx->err[0] = 0;
+    if (!rho_new_host || !J_new_host) { set_err(ctx, "null step pointer", cudaSuccess); return JEFI_ERR_INVALID_ARG; }
+    if (!ctx->has_history) {
+        set_err(ctx, "jefi_append_step before jefi_upload_history", cudaSuccess);
+        return JEFI_ERR_NO_HISTORY;
+    }
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e != cudaSuccess) return cuda_fail(ctx, "cudaSetDevice", e);
+    const size_t plane = (size_t)ctx->P.Ns * ctx->elem;
+    if (!ctx->new_stage) {
+        jefi_status s = dev_alloc(ctx, &ctx->new_stage, 4 * plane, "cudaMalloc(new step staging)");
+        if (s != JEFI_OK) return s;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    char* stage = (char*)ctx->new_stage;
+    if ((e = cudaMemcpyAsync(stage, rho_new_host, plane, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(stage + plane, J_new_host, 3 * plane, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+        return cuda_fail(ctx, "cudaMemcpyAsync(new step)", e);
+    return jefi_append_step(ctx, stage, stage + plane, stream);
 }
 
 jefi_status jefi_upload_history_host(jefi_ctx* ctx, const void* rho_host, const void* J_host,

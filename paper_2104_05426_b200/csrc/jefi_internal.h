@@ -47,6 +47,10 @@ struct FieldsLaunch {
 // leaving the CUDA error in cudaGetLastError()/cudaPeekAtLastError()
 int launch_prepass(const Params& P, jefi_dtype dt, const void* rho, const void* J, void* hist,
                    cudaStream_t stream);
+// sliding window: drop the oldest step, append (rho_new[N_s], J_new[3][N_s]); `last` = raw values
+// of the two newest steps, [2][4][N_s]
+int launch_append(const Params& P, jefi_dtype dt, const void* rho_new, const void* J_new, void* last,
+                  void* hist, cudaStream_t stream);
 int launch_fields_point(const Params& P, jefi_dtype dt, const void* hist, const FieldsLaunch& L);
 // tiled kernel: regular observation grids only; returns 0 if it does not support the request
 int launch_fields_tiled(const Params& P, jefi_dtype dt, const void* hist, const FieldsLaunch& L);

@@ -253,3 +253,86 @@ def test_error_codes_on_device(jb):
         assert ctx.launches > 0
     finally:
         ctx.close()
+
+
+# ------------------------------------------------------------------ sliding window (jefi_append_step)
+def _window(w, lo, T):
+    """The workload restricted to stored steps lo .. lo+T-1 (same arrays, sliced)."""
+    import copy
+    v = copy.copy(w)
+    v.rho = np.ascontiguousarray(w.rho[lo:lo + T])
+    v.J = np.ascontiguousarray(w.J[lo:lo + T])
+    v.T = T
+    return v
+
+
+@pytest.mark.parametrize("dtype,c", [("f64", 1.0), ("f32", 1.0), ("f64", 1.7)])
+@pytest.mark.parametrize("deriv_mode", [0, 1])
+def test_append_step_slides_the_window(jb, dtype, c, deriv_mode):
+    """T stored steps + A appended ones against (i) the oracle on the whole (T+A)-step raw history
+    and (ii) a fresh upload of the last T steps, bit for bit.  The longest lag (k_max = 14 at
+    c = 1) is below T-1 = 19, so neither the dropped steps nor the oldest record's derivative
+    (centred after a slide, one-sided after a fresh upload) is ever read."""
+    import torch
+    T, A = 20, 5
+    full = wl.random_history((6, 5, 4), T + A, seed=41, dtype=dtype, n_obs=(5, 4, 6), dt=0.05, c=c)
+    first = _window(full, 0, T)
+    ctx = make_ctx(first, jb, deriv_mode)
+    try:
+        upload(ctx, first)
+        for a in range(A):
+            rho_new = torch.from_numpy(full.rho[T + a]).cuda()
+            J_new = torch.from_numpy(full.J[T + a]).cuda()
+            if a % 2 == 0:
+                ctx.append_step(rho_new, J_new)
+            else:
+                ctx.append_step_host(torch.from_numpy(full.rho[T + a]).pin_memory(),
+                                     torch.from_numpy(full.J[T + a]).pin_memory())
+            torch.cuda.synchronize()
+            E, B = gpu_fields(ctx, first, T - 1)
+            Eo, Bo = oracle_fields(full, T + a, None, deriv_mode)
+            check(full, E, B, Eo, Bo, None, f"after {a + 1} appends")
+        fresh_w = _window(full, A, T)
+        fresh = make_ctx(fresh_w, jb, deriv_mode)
+        try:
+            upload(fresh, fresh_w)
+            for kernel in KERNELS:
+                ctx.set_kernel(kernel); fresh.set_kernel(kernel)
+                E2, B2 = gpu_fields(fresh, fresh_w, T - 1)
+                E1, B1 = gpu_fields(ctx, first, T - 1)
+                np.testing.assert_array_equal(E1, E2)
+                np.testing.assert_array_equal(B1, B2)
+            # jefi_fields_at_time follows the advanced t0
+            Ed = torch.empty((3, full.N_o), dtype=torch.float64 if dtype == "f64" else torch.float32, device="cuda")
+            Bd = torch.empty_like(Ed)
+            jb.jefi_fields_at_time(ctx.ctx, (T - 1 + A) * full.dt, 0, full.N_o, Ed, Bd)
+            torch.cuda.synchronize()
+            np.testing.assert_array_equal(Ed.cpu().numpy().astype(np.float64), E1)
+        finally:
+            fresh.close()
+    finally:
+        ctx.close()
+
+
+def test_append_step_single_stored_step_and_errors(jb):
+    import torch
+    w = wl.random_history((3, 3, 2), 3, seed=43, dtype="f64", n_obs=(2, 2, 2), spacing_obs=(0.01, 0.01, 0.01),
+                          origin_obs=(0.4, 0.0, 0.0), dt=10.0)
+    one = _window(w, 0, 1)
+    ctx = make_ctx(one, jb)
+    try:
+        with pytest.raises(jb.JefiError) as e:
+            ctx.append_step(torch.from_numpy(w.rho[1]).cuda(), torch.from_numpy(w.J[1]).cuda())
+        assert e.value.status == jb.JEFI_ERR_NO_HISTORY
+        upload(ctx, one)
+        with pytest.raises(jb.JefiError) as e:
+            jb.jefi_append_step(ctx.ctx, None, torch.from_numpy(w.J[1]).cuda())
+        assert e.value.status == jb.JEFI_ERR_INVALID_ARG
+        # T = 1: every lag is 0 (dt = 10), the stored step is replaced and gets (f_new - f_prev)/dt
+        for a in (1, 2):
+            ctx.append_step(torch.from_numpy(w.rho[a]).cuda(), torch.from_numpy(w.J[a]).cuda())
+            E, B = gpu_fields(ctx, one, 0)
+            Eo, Bo = oracle_fields(_window(w, 0, a + 1), a, None, 1)     # backward difference == one-sided
+            check(w, E, B, Eo, Bo, None, f"T=1 after {a} appends")
+    finally:
+        ctx.close()
