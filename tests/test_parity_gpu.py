@@ -336,3 +336,56 @@ def test_append_step_single_stored_step_and_errors(jb):
             check(w, E, B, Eo, Bo, None, f"T=1 after {a} appends")
     finally:
         ctx.close()
+
+
+# ------------------------------------------------------------------ long retarded-time windows
+@pytest.mark.parametrize("dtype,kernel", [("f32", 2), ("f64", 0)])
+def test_long_windows_use_the_widest_tile_variant(jb, dtype, kernel):
+    """dx/(c dt) = 20: a tile's lag window is ~250 steps -> fp32 takes the 512-slot shared-memory
+    variant (one CTA per SM; kernel 2 = tiled or JEFI_ERR_UNSUPPORTED), fp64 (64-byte records) no
+    longer fits and falls back to the per-point kernel.  The history (T = 300) is shorter than
+    the longest lag (~500).  Geometry: offsets are half-integer multiples of dx on two axes, so
+    no pair sits on the screening radius and q = 10 sqrt(N) stays >= 5e-4 away from a tie."""
+    w = wl.random_history((5, 4, 3), 300, seed=51, dtype=dtype, n_obs=(10, 8, 8), dt=0.005)
+    ctx = make_ctx(w, jb)
+    try:
+        ctx.set_kernel(kernel)
+        upload(ctx, w)
+        for n in (299, 120, 7):
+            E, B = gpu_fields(ctx, w, n)
+            Eo, Bo = oracle_fields(w, n)
+            check(w, E, B, Eo, Bo, None, f"long window step {n}")
+    finally:
+        ctx.close()
+
+
+def test_windows_beyond_shared_memory_fall_back_to_the_point_kernel(jb):
+    """dx/(c dt) = 50: ~610-step windows do not fit; automatic selection uses the per-point
+    kernel, forcing the tiled kernel is refused."""
+    import torch
+    w = wl.random_history((4, 4, 3), 64, seed=53, dtype="f64", n_obs=(9, 8, 8), dt=0.002)
+    ctx = make_ctx(w, jb)
+    try:
+        upload(ctx, w)
+        E, B = gpu_fields(ctx, w, 63)
+        Eo, Bo = oracle_fields(w, 63)
+        check(w, E, B, Eo, Bo, None, "fallback")
+        ctx.set_kernel(2)
+        Ed = torch.empty((3, w.N_o), dtype=torch.float64, device="cuda")
+        with pytest.raises(jb.JefiError) as e:
+            ctx.fields(63, Ed, torch.empty_like(Ed))
+        assert e.value.status == jb.JEFI_ERR_UNSUPPORTED
+    finally:
+        ctx.close()
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("n_obs", [(12, 9, 10), (4, 20, 3), (20, 12, 1), (33, 16, 2)])
+def test_ragged_tiles_every_edge_shape(jb, dtype, n_obs):
+    """Observation grids that end inside a tile in x (half-x variant), y (warps along y), z (idle
+    warps), all three, and plane-shaped sets; full oracle comparison.  Same spacing as the
+    source grid: offsets are integer on all axes or half-integer on two, so no pair sits on the
+    screening radius (R = dx/2 needs exactly one half-integer axis) and q = 2 sqrt(M) or sqrt(N)
+    stays >= 1.5e-3 away from a rounding tie (white-noise history: a flipped index would show)."""
+    w = wl.random_history((6, 5, 4), 48, seed=57, dtype=dtype, n_obs=n_obs, dt=0.05)
+    run_case(jb, w, None, 2, steps=(47, 11))
