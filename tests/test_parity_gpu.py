@@ -16,6 +16,8 @@ KERNELS = [1, 0]        # 1 = per-point kernel, 0 = automatic (tiled where suppo
 
 @pytest.fixture(scope="module")
 def jb():
+    import __graft_entry__
+    __graft_entry__.build()            # no-op when libjefi.so is newer than its sources
     import paper_2104_05426_b200 as jb
     return jb
 
@@ -339,11 +341,10 @@ def test_append_step_single_stored_step_and_errors(jb):
 
 
 # ------------------------------------------------------------------ long retarded-time windows
-@pytest.mark.parametrize("dtype,kernel", [("f32", 2), ("f64", 0)])
+@pytest.mark.parametrize("dtype,kernel", [("f32", 2), ("f64", 2)])
 def test_long_windows_use_the_widest_tile_variant(jb, dtype, kernel):
-    """dx/(c dt) = 20: a tile's lag window is ~250 steps -> fp32 takes the 512-slot shared-memory
-    variant (one CTA per SM; kernel 2 = tiled or JEFI_ERR_UNSUPPORTED), fp64 (64-byte records) no
-    longer fits and falls back to the per-point kernel.  The history (T = 300) is shorter than
+    """dx/(c dt) = 20: a tile's lag window is ~250 steps -> the 512-slot shared-memory variant,
+    one CTA per SM (fp64: two cells per stage); kernel 2 = tiled or JEFI_ERR_UNSUPPORTED.  The history (T = 300) is shorter than
     the longest lag (~500).  Geometry: offsets are half-integer multiples of dx on two axes, so
     no pair sits on the screening radius and q = 10 sqrt(N) stays >= 5e-4 away from a tie."""
     w = wl.random_history((5, 4, 3), 300, seed=51, dtype=dtype, n_obs=(10, 8, 8), dt=0.005)
