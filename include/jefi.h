@@ -78,10 +78,10 @@ typedef struct {
 } jefi_time_desc;
 
 /* Validates the descriptors, selects `device`, and allocates everything the context will
- * ever need on it: the packed history (2 x 16-byte (fp32) / 2 x 32-byte (fp64) half-records
- * per (cell, step), plus one all-zero step for m < 0), partial-sum scratch, and the device
- * output staging used by jefi_fields_host.  No kernel is launched.  *out is written only on
- * success.  Synchronous. */
+ * ever need on it: the packed history (32 bytes (fp32) / 64 bytes (fp64) per (cell, step), plus
+ * one all-zero step standing for m < 0), the raw values of the two newest steps (for
+ * jefi_append_step), partial-sum scratch, and the device output staging used by
+ * jefi_fields_host.  No kernel is launched.  *out is written only on success.  Synchronous. */
 jefi_status jefi_create(const jefi_grid_desc* src, const jefi_obs_desc* obs,
                         const jefi_time_desc* time, jefi_dtype dtype, int device,
                         jefi_ctx** out);
