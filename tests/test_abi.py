@@ -83,6 +83,33 @@ def test_create_rejects_null_and_bad_dtype(jb):
         assert e.value.status == jb.JEFI_ERR_INVALID_ARG
 
 
+def test_create_refuses_sizes_beyond_the_index_range(jb):
+    """2^31 source cells exceed the 32-bit cell index of the kernels: refused before any
+    allocation (JEFI_ERR_UNSUPPORTED), as is an observation set of 2^40 points."""
+    src, obs, tm = _descs(jb, n=(2048, 2048, 512))
+    obs.grid = jb.make_grid((4, 4, 4), (0, 0, 0), (0.1, 0.1, 0.1))
+    with pytest.raises(jb.JefiError) as e:
+        jb.jefi_create(src, obs, tm, jb.JEFI_F32, 0)
+    assert e.value.status == jb.JEFI_ERR_UNSUPPORTED
+    src, obs, tm = _descs(jb)
+    pts = jb.jefi_obs_desc()
+    pts.kind, pts.npoints, pts.points_dev = 1, 1 << 40, 16
+    pts.grid = jb.make_grid((1, 1, 1), (0, 0, 0), (1, 1, 1))
+    with pytest.raises(jb.JefiError) as e:
+        jb.jefi_create(src, pts, tm, jb.JEFI_F32, 0)
+    assert e.value.status == jb.JEFI_ERR_UNSUPPORTED
+
+
+def test_append_and_shard_reject_null_arguments(jb):
+    lib = C.CDLL(str(jb.LIB_PATH))
+    lib.jefi_append_step.argtypes = [C.c_void_p] * 4
+    lib.jefi_append_step_host.argtypes = [C.c_void_p] * 4
+    assert lib.jefi_append_step(None, None, None, None) == jb.JEFI_ERR_INVALID_ARG
+    assert lib.jefi_append_step_host(None, None, None, None) == jb.JEFI_ERR_INVALID_ARG
+    lib.jefi_shard_obs.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
+    assert lib.jefi_shard_obs(None, 0, 1, None, None) == jb.JEFI_ERR_INVALID_ARG
+
+
 def test_null_context_is_an_error_not_a_crash(jb):
     lib = C.CDLL(str(jb.LIB_PATH))
     lib.jefi_fields.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
