@@ -38,8 +38,10 @@ constexpr int kCells2 = 128;
 template <typename T, int TT>
 __global__ void __launch_bounds__(kThreads)
 prepass_march_kernel(const T* __restrict__ rho, const T* __restrict__ J, Unit<T>* __restrict__ hist,
-                     long long Ns, int Tsteps, int Tp, T inv_dt, T inv_c, int deriv_mode)
+                     long long Ns, int Tsteps, int Tp, T inv_dt, T inv_c, int deriv_mode, int seg_len)
 {
+    // blockIdx.y = time segment: packed steps [seg_len * blockIdx.y, + seg_len), seg_len a multiple
+    // of TT (several segments only to have enough CTAs for full waves; each re-reads two rows)
     // raw[comp][row][cell(+1 pad)], row r <-> stored step m = p0 - 2 + r
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T (*raw)[TT + 2][kCells2 + 1] = reinterpret_cast<T (*)[TT + 2][kCells2 + 1]>(smem_raw);
@@ -49,10 +51,19 @@ prepass_march_kernel(const T* __restrict__ rho, const T* __restrict__ J, Unit<T>
     constexpr int U = sizeof(T) == 4 ? 2 : 4, VPU = 8 / U;
     const T half = T(0.5), ic = inv_c, ic2 = inv_c * inv_c;
 
-    for (int i = threadIdx.x; i < 4 * 2 * kCells2; i += kThreads)
-        raw[i / (2 * kCells2)][(i / kCells2) % 2][i % kCells2] = T(0);
+    const int p_begin = (int)blockIdx.y * seg_len;
+    const int p_end = p_begin + seg_len < Tp ? p_begin + seg_len : Tp;
+    for (int i = threadIdx.x; i < 4 * 2 * kCells2; i += kThreads) {
+        const int comp = i / (2 * kCells2), r = (i / kCells2) % 2, cl = i % kCells2;
+        const int m = p_begin - 2 + r;
+        const long long j = j0 + cl;
+        T v = T(0);
+        if (m >= 0 && m < Tsteps && j < Ns)
+            v = (comp == 0) ? rho[(long long)m * Ns + j] : J[((long long)m * 3 + (comp - 1)) * Ns + j];
+        raw[comp][r][cl] = v;
+    }
 
-    for (int p0 = 0; p0 < Tp; p0 += TT) {
+    for (int p0 = p_begin; p0 < p_end; p0 += TT) {
         for (int row = warp; row < 4 * TT; row += kThreads / 32) {
             const int comp = row / TT, r = 2 + row % TT;
             const int m = p0 - 2 + r;
@@ -182,18 +193,29 @@ int launch_prepass(const Params& P, jefi_dtype dt, const void* rho, const void* 
 {
     const unsigned blocks = (unsigned)((P.Ns + kCells2 - 1) / kCells2);
     constexpr int TT = 16;
+    // time segments: aim at >= 8 waves of CTAs (a CTA marches through its whole segment, so a
+    // partial last wave costs up to one CTA's run time)
+    int sm_count = 148, dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
+    const int tiles_t = (P.Tp + TT - 1) / TT;
+    long long want = (8LL * sm_count * 6 + blocks - 1) / blocks;
+    if (want < 1) want = 1;
+    if (want > tiles_t) want = tiles_t;
+    const int seg_tiles = (int)((tiles_t + want - 1) / want);
+    const int seg_len = seg_tiles * TT;
+    const dim3 grid(blocks, (unsigned)((tiles_t + seg_tiles - 1) / seg_tiles));
     if (dt == JEFI_F32) {
         const int smem = 4 * (TT + 2) * (kCells2 + 1) * (int)sizeof(float);
         auto kern = prepass_march_kernel<float, TT>;
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return -1;
-        kern<<<blocks, kThreads, smem, stream>>>((const float*)rho, (const float*)J, (Unit<float>*)hist, P.Ns, P.T,
-                                                 P.Tp, (float)(1.0 / P.dt), (float)(1.0 / P.c), P.deriv_mode);
+        kern<<<grid, kThreads, smem, stream>>>((const float*)rho, (const float*)J, (Unit<float>*)hist, P.Ns, P.T,
+                                               P.Tp, (float)(1.0 / P.dt), (float)(1.0 / P.c), P.deriv_mode, seg_len);
     } else {
         const int smem = 4 * (TT + 2) * (kCells2 + 1) * (int)sizeof(double);
         auto kern = prepass_march_kernel<double, TT>;
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return -1;
-        kern<<<blocks, kThreads, smem, stream>>>((const double*)rho, (const double*)J, (Unit<double>*)hist, P.Ns, P.T,
-                                                 P.Tp, 1.0 / P.dt, 1.0 / P.c, P.deriv_mode);
+        kern<<<grid, kThreads, smem, stream>>>((const double*)rho, (const double*)J, (Unit<double>*)hist, P.Ns, P.T,
+                                               P.Tp, 1.0 / P.dt, 1.0 / P.c, P.deriv_mode, seg_len);
     }
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
