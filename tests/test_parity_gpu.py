@@ -417,3 +417,43 @@ def test_full_size_every_point_tiled_vs_point_kernel(jb, make, step):
             assert max(rel_l2(got, ref, field_ref=ref)) <= 4e-4
     finally:
         ctx.close()
+
+
+# ------------------------------------------------------------------ the paper's own test case (Sec. 3.1)
+def test_paper_constant_sources_410_snapshots(jb):
+    """PAPER.md:122-139, :213-219 (Table 2): rho = 1, J = (1,1,1) switched on at t = 0 on the 15^3
+    grid over [-3,3]^3, 410 snapshots at dt = 0.05, fp32 storage.  All 411 steps through the C
+    ABI; seven of them against the oracle on every point; the legend magnitude of Fig. 4/5 at
+    t = 2.5 (~0.5); and the paper's saturation (after the longest
+    light-travel time the fields no longer change) bit for bit on the CUDA output."""
+    import time
+    import torch
+    T = 411
+    w = wl.paper_x1_constant(T, n=15, dtype="f32")
+    ctx = make_ctx(w, jb)
+    try:
+        upload(ctx, w)
+        E = torch.empty((T, 3, w.N_o), dtype=torch.float32, device="cuda")
+        B = torch.empty_like(E)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for n in range(T):
+            ctx.fields(n, E[n], B[n])
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        E, B = E.cpu().numpy().astype(np.float64), B.cpu().numpy().astype(np.float64)
+        for n in (0, 1, 50, 100, 150, 250, 410):
+            Eo, Bo = oracle_fields(w, n)
+            check(w, E[n], B[n], Eo, Bo, None, f"paper X1 step {n}")
+        plane = np.arange(15 * 15) + 7 * 15 * 15                     # the z = 0 layer
+        e_max = np.sqrt(E[50][0][plane] ** 2 + E[50][1][plane] ** 2).max()
+        b_max = np.sqrt(B[50][0][plane] ** 2 + B[50][1][plane] ** 2).max()
+        assert abs(e_max - 0.529) < 2e-3 and abs(b_max - 0.529) < 2e-3
+        k_max = int(np.floor(np.sqrt(3.0) * 14 * 0.4 / 0.05 + 0.5))  # longest lag on the grid: 194
+        for n in range(k_max + 2, T):
+            assert np.array_equal(E[n], E[T - 1]) and np.array_equal(B[n], B[T - 1]), n
+        assert not np.array_equal(E[k_max - 20], E[T - 1])
+        print(f"\npaper Table 2 workload: 411 snapshots of [15^3,15^3] in {wall * 1e3:.1f} ms wall "
+              f"({wall / T * 1e6:.0f} us per snapshot; the paper: 8.696 s on a Tesla V100, PAPER.md:217)")
+    finally:
+        ctx.close()
