@@ -178,10 +178,12 @@ jefi_status jefi_create(const jefi_grid_desc* src, const jefi_obs_desc* obs,
     if (e != cudaSuccess) { cudaGetLastError(); delete c; return JEFI_ERR_CUDA; }
     c->sm_count = prop.multiProcessorCount;
 
-    // scratch: partial sums [S chunks][6 components][points] in double.  Room for 16 chunks of the
-    // whole observation set (capped at 1 GiB, never below one chunk); the launchers choose S to fit.
-    long long pts = P.n_obs < 32768 ? 32768 : P.n_obs;
-    long long elems = 6 * 16 * pts;
+    // scratch: partial sums [S chunks][6 components][points] in double.  Room for 64 chunks of the
+    // whole observation set (capped at 1 GiB, never below one chunk), so that the launchers can
+    // pick a chunk count that fills the last wave of CTAs; more chunks than fit go to further,
+    // accumulating launches.
+    long long pts = P.n_obs < 8192 ? 8192 : P.n_obs;
+    long long elems = 6 * 64 * pts;
     if (elems > (1LL << 27)) elems = (1LL << 27);
     if (elems < 6 * P.n_obs) elems = 6 * P.n_obs;
     c->scratch_elems = elems;
