@@ -130,6 +130,15 @@ jefi_status jefi_append_step_host(jefi_ctx* ctx, const void* rho_new_host, const
 jefi_status jefi_fields(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t obs_count,
                         void* E_out_dev, void* B_out_dev, jefi_stream stream);
 
+/* A time series in one call (the paper evaluates hundreds of snapshots on fixed grids,
+ * PAPER.md:213-219; BASELINE.json configs[3] asks for 128 output steps): the same as
+ * step_count calls of jefi_fields for step_begin, step_begin+1, ... with outputs
+ * E_out_dev[step_count][3][obs_count], B_out_dev likewise.  All launches are enqueued on
+ * `stream` back to back; step_count = 0 is a no-op. */
+jefi_status jefi_fields_series(jefi_ctx* ctx, int32_t step_begin, int32_t step_count,
+                               int64_t obs_begin, int64_t obs_count,
+                               void* E_out_dev, void* B_out_dev, jefi_stream stream);
+
 /* Same for a time t that must lie on the step grid to within 1e-6*dt (the paper
  * evaluates at snapshots only), else JEFI_ERR_TIME_RANGE. */
 jefi_status jefi_fields_at_time(jefi_ctx* ctx, double t, int64_t obs_begin, int64_t obs_count,

@@ -24,7 +24,7 @@ EXPORTS = (
     "jefi_fields_at_time", "jefi_fields_host", "jefi_set_kernel", "jefi_launch_count",
     "jefi_device_bytes", "jefi_destroy", "jefi_status_string", "jefi_last_error",
     "jefi_flops_per_pair", "jefi_measure_alu_peak", "jefi_shard_obs",
-    "jefi_append_step", "jefi_append_step_host",
+    "jefi_append_step", "jefi_append_step_host", "jefi_fields_series",
 )
 
 
@@ -63,6 +63,7 @@ _lib.jefi_upload_history_host.argtypes = [_P, _P, _P, _P]
 _lib.jefi_append_step.argtypes = [_P, _P, _P, _P]
 _lib.jefi_append_step_host.argtypes = [_P, _P, _P, _P]
 _lib.jefi_fields.argtypes = [_P, C.c_int32, C.c_int64, C.c_int64, _P, _P, _P]
+_lib.jefi_fields_series.argtypes = [_P, C.c_int32, C.c_int32, C.c_int64, C.c_int64, _P, _P, _P]
 _lib.jefi_fields_at_time.argtypes = [_P, C.c_double, C.c_int64, C.c_int64, _P, _P, _P]
 _lib.jefi_fields_host.argtypes = [_P, C.c_int32, C.c_int64, C.c_int64, _P, _P, _P]
 _lib.jefi_set_kernel.argtypes = [_P, C.c_int32]
@@ -162,6 +163,11 @@ def jefi_fields(ctx, step, obs_begin, obs_count, E_out_dev, B_out_dev, stream=No
                             _stream(stream)), ctx, "jefi_fields")
 
 
+def jefi_fields_series(ctx, step_begin, step_count, obs_begin, obs_count, E_out_dev, B_out_dev, stream=None):
+    _check(_lib.jefi_fields_series(ctx, int(step_begin), int(step_count), int(obs_begin), int(obs_count),
+                                   _ptr(E_out_dev), _ptr(B_out_dev), _stream(stream)), ctx, "jefi_fields_series")
+
+
 def jefi_fields_at_time(ctx, t, obs_begin, obs_count, E_out_dev, B_out_dev, stream=None):
     _check(_lib.jefi_fields_at_time(ctx, float(t), int(obs_begin), int(obs_count), _ptr(E_out_dev),
                                     _ptr(B_out_dev), _stream(stream)), ctx, "jefi_fields_at_time")
@@ -255,6 +261,10 @@ class Jefi:
     def fields(self, step, E_out_dev, B_out_dev, obs_begin=0, obs_count=None, stream=None):
         n = self.n_points - obs_begin if obs_count is None else obs_count
         jefi_fields(self.ctx, step, obs_begin, n, E_out_dev, B_out_dev, stream)
+
+    def fields_series(self, step_begin, step_count, E_out_dev, B_out_dev, obs_begin=0, obs_count=None, stream=None):
+        n = self.n_points - obs_begin if obs_count is None else obs_count
+        jefi_fields_series(self.ctx, step_begin, step_count, obs_begin, n, E_out_dev, B_out_dev, stream)
 
     def fields_host(self, step, E_out_host, B_out_host, obs_begin=0, obs_count=None, stream=None):
         n = self.n_points - obs_begin if obs_count is None else obs_count

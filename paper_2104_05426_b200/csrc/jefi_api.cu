@@ -329,6 +329,27 @@ jefi_status jefi_fields(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t 
     return run_fields(ctx, step, obs_begin, obs_count, E_out_dev, B_out_dev, (cudaStream_t)stream);
 }
 
+jefi_status jefi_fields_series(jefi_ctx* ctx, int32_t step_begin, int32_t step_count,
+                               int64_t obs_begin, int64_t obs_count,
+                               void* E_out_dev, void* B_out_dev, jefi_stream stream)
+{
+    if (!ctx) return JEFI_ERR_INVALID_ARG;
+    if (step_count < 0) { set_err(ctx, "negative step count", cudaSuccess); return JEFI_ERR_INVALID_ARG; }
+    if (step_count == 0) return JEFI_OK;
+    // every argument is checked before the first launch
+    jefi_status s = check_fields_args(ctx, step_begin, obs_begin, obs_count, E_out_dev, B_out_dev);
+    if (s != JEFI_OK) return s;
+    s = check_fields_args(ctx, step_begin + step_count - 1, obs_begin, obs_count, E_out_dev, B_out_dev);
+    if (s != JEFI_OK) return s;
+    const size_t stride = (size_t)obs_count * 3 * ctx->elem;
+    for (int32_t k = 0; k < step_count; ++k) {
+        s = run_fields(ctx, step_begin + k, obs_begin, obs_count, (char*)E_out_dev + (size_t)k * stride,
+                       (char*)B_out_dev + (size_t)k * stride, (cudaStream_t)stream);
+        if (s != JEFI_OK) return s;
+    }
+    return JEFI_OK;
+}
+
 jefi_status jefi_fields_at_time(jefi_ctx* ctx, double t, int64_t obs_begin, int64_t obs_count,
                                 void* E_out_dev, void* B_out_dev, jefi_stream stream)
 {

@@ -119,21 +119,31 @@ fields_point_kernel(const T* __restrict__ hist, double* __restrict__ partial, Po
     for (int c = 0; c < 6; ++c) out[(long long)c * a.obs_count] = tot[c];
 }
 
-// step a6: fixed-order sum over the S source chunks, scale, store as component planes
+// step a6: fixed-order sum over the S source chunks, scale, store as component planes.
+// One thread per (component, point); the S loads of a thread are independent (eight in flight).
 template <typename T>
 __global__ void __launch_bounds__(256)
 reduce_scale_kernel(const double* __restrict__ partial, T* __restrict__ E, T* __restrict__ B,
                     long long count, int S, double scaleE, double scaleB)
 {
-    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
-    if (i >= count) return;
+    const long long t = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (t >= 6 * count) return;
+    const int c = (int)(t / count);
+    const long long i = t - (long long)c * count;
+    const double* src = partial + (long long)c * count + i;
+    const long long stride = 6 * count;
+    double acc = 0.0;
+    int s = 0;
+    for (; s + 8 <= S; s += 8) {
+        double v[8];
 #pragma unroll
-    for (int c = 0; c < 6; ++c) {
-        double acc = 0.0;
-        for (int s = 0; s < S; ++s) acc += partial[((long long)s * 6 + c) * count + i];
-        if (c < 3) E[(long long)c * count + i] = (T)(acc * scaleE);
-        else       B[(long long)(c - 3) * count + i] = (T)(acc * scaleB);
+        for (int e = 0; e < 8; ++e) v[e] = src[(long long)(s + e) * stride];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) acc += v[e];          // same order as a plain loop over s
     }
+    for (; s < S; ++s) acc += src[(long long)s * stride];
+    if (c < 3) E[(long long)c * count + i] = (T)(acc * scaleE);
+    else       B[(long long)(c - 3) * count + i] = (T)(acc * scaleB);
 }
 
 }  // namespace
@@ -143,7 +153,7 @@ int launch_reduce_scale(const Params& P, jefi_dtype dt, const FieldsLaunch& L, i
     const double pi = 3.14159265358979323846;
     const double dV = P.sh[0] * P.sh[1] * P.sh[2];
     const double scaleE = dV / (4.0 * pi), scaleB = P.c * scaleE;
-    const unsigned grid = (unsigned)((L.obs_count + 255) / 256);
+    const unsigned grid = (unsigned)((6 * L.obs_count + 255) / 256);
     if (dt == JEFI_F32)
         reduce_scale_kernel<float><<<grid, 256, 0, L.stream>>>(
             (const double*)L.scratch, (float*)L.E_out, (float*)L.B_out, L.obs_count, S, scaleE, scaleB);

@@ -343,8 +343,8 @@ def test_append_step_single_stored_step_and_errors(jb):
 # ------------------------------------------------------------------ long retarded-time windows
 @pytest.mark.parametrize("dtype,kernel", [("f32", 2), ("f64", 2)])
 def test_long_windows_use_the_widest_tile_variant(jb, dtype, kernel):
-    """dx/(c dt) = 20: a tile's lag window is ~250 steps -> the 512-slot shared-memory variant,
-    one CTA per SM (fp64: two cells per stage); kernel 2 = tiled or JEFI_ERR_UNSUPPORTED.  The history (T = 300) is shorter than
+    """dx/(c dt) = 20: a tile's lag window is ~250 steps -> the kernel variant whose window
+    capacity comes from the launch, one CTA per SM; kernel 2 = tiled or JEFI_ERR_UNSUPPORTED.  The history (T = 300) is shorter than
     the longest lag (~500).  Geometry: offsets are half-integer multiples of dx on two axes, so
     no pair sits on the screening radius and q = 10 sqrt(N) stays >= 5e-4 away from a tie."""
     w = wl.random_history((5, 4, 3), 300, seed=51, dtype=dtype, n_obs=(10, 8, 8), dt=0.005)
@@ -361,10 +361,10 @@ def test_long_windows_use_the_widest_tile_variant(jb, dtype, kernel):
 
 
 def test_windows_beyond_shared_memory_fall_back_to_the_point_kernel(jb):
-    """dx/(c dt) = 50: ~610-step windows do not fit; automatic selection uses the per-point
-    kernel, forcing the tiled kernel is refused."""
+    """dx/(c dt) = 500: ~6000-step windows (384 KB per cell in fp64) do not fit in shared memory;
+    automatic selection uses the per-point kernel, forcing the tiled kernel is refused."""
     import torch
-    w = wl.random_history((4, 4, 3), 64, seed=53, dtype="f64", n_obs=(9, 8, 8), dt=0.002)
+    w = wl.random_history((4, 4, 3), 64, seed=53, dtype="f64", n_obs=(9, 8, 8), dt=0.0002)
     ctx = make_ctx(w, jb)
     try:
         upload(ctx, w)
@@ -437,10 +437,18 @@ def test_paper_constant_sources_410_snapshots(jb):
         B = torch.empty_like(E)
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        for n in range(T):
-            ctx.fields(n, E[n], B[n])
+        ctx.fields_series(0, T, E, B)                      # one C call, 411 evaluations
         torch.cuda.synchronize()
         wall = time.perf_counter() - t0
+        E1 = torch.empty((3, w.N_o), dtype=torch.float32, device="cuda")
+        B1 = torch.empty_like(E1)
+        for n in (0, 77, 410):                             # the series equals the single calls
+            ctx.fields(n, E1, B1)
+            torch.cuda.synchronize()
+            assert torch.equal(E1, E[n]) and torch.equal(B1, B[n])
+        with pytest.raises(jb.JefiError) as e:
+            ctx.fields_series(400, 20, E, B)
+        assert e.value.status == jb.JEFI_ERR_TIME_RANGE
         E, B = E.cpu().numpy().astype(np.float64), B.cpu().numpy().astype(np.float64)
         for n in (0, 1, 50, 100, 150, 250, 410):
             Eo, Bo = oracle_fields(w, n)
