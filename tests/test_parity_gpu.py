@@ -465,3 +465,49 @@ def test_paper_constant_sources_410_snapshots(jb):
               f"({wall / T * 1e6:.0f} us per snapshot; the paper: 8.696 s on a Tesla V100, PAPER.md:217)")
     finally:
         ctx.close()
+
+
+# ------------------------------------------------------------------ seeded fuzz of the launch logic
+def test_fuzz_random_geometries_fp64(jb):
+    """150 seeded random set-ups (grid shapes, anisotropic spacings, offsets, c, dt from
+    dx/(c dt) = 0.5 to 12, history lengths from 1 step to beyond the longest lag, evaluation step,
+    observation sub-range, derivative mode) through the tiled kernel in fp64, each against the
+    oracle on every requested point.  Exercises tile raggedness, window capacities (32 / 96 /
+    sized by the launch), zero-filled pre-history slots, chunking and sub-range clipping in
+    combinations the named cases do not.  fp64 and real-valued geometry: a rounding tie or a pair
+    on the screening radius has measure zero."""
+    import torch
+    rng = np.random.default_rng(20210405)
+    ran = 0
+    for case in range(150):
+        n_src = tuple(int(v) for v in rng.integers(1, 13, 3))
+        n_obs = tuple(int(v) for v in rng.integers(1, 21, 3))
+        sp_src = tuple(float(v) for v in rng.uniform(0.05, 0.3, 3))
+        sp_obs = tuple(float(v) for v in rng.uniform(0.05, 0.3, 3))
+        origin_obs = tuple(float(-(n - 1) / 2 * h + rng.uniform(-0.5, 0.5)) for n, h in zip(n_obs, sp_obs))
+        c = float(rng.uniform(0.5, 2.0))
+        dt = float(min(sp_src) / (c * rng.uniform(0.5, 12.0)))
+        T = int(rng.integers(1, 81))
+        w = wl.random_history(n_src, T, seed=1000 + case, dtype="f64", spacing=sp_src, n_obs=n_obs,
+                              spacing_obs=sp_obs, origin_obs=origin_obs, dt=dt, c=c)
+        step = int(rng.integers(0, T))
+        begin = int(rng.integers(0, w.N_o))
+        count = int(rng.integers(1, w.N_o - begin + 1))
+        mode = int(rng.integers(0, 2))
+        ctx = make_ctx(w, jb, mode)
+        try:
+            ctx.set_kernel(2)
+            upload(ctx, w)
+            try:
+                E, B = gpu_fields(ctx, w, step, begin, count)
+            except jb.JefiError as e:                      # window beyond shared memory
+                assert e.status == jb.JEFI_ERR_UNSUPPORTED
+                continue
+            idx = np.arange(begin, begin + count)
+            Eo, Bo = oracle_fields(w, step, idx, mode)
+            check(w, E, B, Eo, Bo, None, f"fuzz case {case}: src {n_src} obs {n_obs} T {T} step {step} "
+                                          f"range {begin}+{count} mode {mode} dx/cdt {min(sp_src) / (c * dt):.2f}")
+            ran += 1
+        finally:
+            ctx.close()
+    assert ran >= 120
