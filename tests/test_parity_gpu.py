@@ -511,3 +511,37 @@ def test_fuzz_random_geometries_fp64(jb):
         finally:
             ctx.close()
     assert ran >= 120
+
+
+def test_fuzz_random_lattices_fp32(jb):
+    """The same for fp32 on white-noise histories, where one flipped retarded index is an O(1)
+    error in its term: 80 seeded random shapes on commensurate lattices (equal spacing,
+    dx/(c dt) in {1, 2, 4}, centred grids whose offsets are integer on all axes or half-integer
+    on at least two, so that no lag is a rounding tie -- 4M = odd square is impossible mod 4 / mod
+    8 -- and no pair sits on the screening radius)."""
+    rng = np.random.default_rng(5426)
+    ran = 0
+    while ran < 80:
+        n_src = tuple(int(v) for v in rng.integers(1, 13, 3))
+        n_obs = tuple(int(v) for v in rng.integers(1, 21, 3))
+        if sum((a - b) % 2 for a, b in zip(n_src, n_obs)) == 1:
+            continue                                       # exactly one half-cell offset: R can equal rcut
+        ratio = int(rng.choice([1, 2, 4]))
+        T = int(rng.integers(1, 81))
+        w = wl.random_history(n_src, T, seed=3000 + ran, dtype="f32", n_obs=n_obs, dt=0.1 / ratio)
+        step = int(rng.integers(0, T))
+        begin = int(rng.integers(0, w.N_o))
+        count = int(rng.integers(1, w.N_o - begin + 1))
+        mode = int(rng.integers(0, 2))
+        ctx = make_ctx(w, jb, mode)
+        try:
+            ctx.set_kernel(2)
+            upload(ctx, w)
+            E, B = gpu_fields(ctx, w, step, begin, count)
+            idx = np.arange(begin, begin + count)
+            Eo, Bo = oracle_fields(w, step, idx, mode)
+            check(w, E, B, Eo, Bo, None, f"fp32 fuzz {ran}: src {n_src} obs {n_obs} T {T} step {step} "
+                                          f"range {begin}+{count} mode {mode} dx/cdt {ratio}")
+            ran += 1
+        finally:
+            ctx.close()
