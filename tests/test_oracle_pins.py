@@ -431,3 +431,112 @@ def test_argument_validation():
         oracle.fields(w.n_src, w.origin_src, w.spacing_src, w.rho, w.J, dt=w.dt, c=1.0, step=4, obs_xyz=[(0, 0, 1)])
     with pytest.raises(ValueError):
         oracle.fields(w.n_src, w.origin_src, w.spacing_src, w.rho, w.J, dt=-1.0, c=1.0, step=0, obs_xyz=[(0, 0, 1)])
+
+
+# --------------------------------------------------------------------------- derivative ends, T = 1, tie direction
+def _one_cell_nonlinear(T):
+    """One source cell at the origin (grid 1x1x1, spacing 0.1: dV = 1e-3, rcut = 0.05) with a
+    history that is NOT linear in the step index, so that a centred, a one-sided and a
+    half-weighted one-sided difference all give different numbers:
+        rho[m] = m^2 + 1,    J[m] = (m^3, -2 m^2, 3 m + m^2)."""
+    m = np.arange(T, dtype=np.float64)
+    rho = (m * m + 1.0).reshape(T, 1, 1, 1)
+    J = np.stack([m ** 3, -2.0 * m * m, 3.0 * m + m * m], axis=1).reshape(T, 3, 1, 1, 1)
+    return rho, J
+
+
+def _one_cell_expect(dvec, c, rho_m, rhod, J_m, Jd, dV=1e-3):
+    """Eq. (4)-(5) for ONE cell, written out: the closed form the pins below
+    compare with.  rho_m, J_m = stored values at the retarded step, rhod, Jd = the time
+    derivative SURVEY.md 8c's definition of D prescribes there (worked out by hand per test)."""
+    d = np.asarray(dvec, dtype=np.float64)
+    R = float(np.linalg.norm(d))
+    E = d * (rho_m / R ** 3 + rhod / (c * R ** 2)) - np.asarray(Jd) / (c * c * R)
+    B = np.cross(np.asarray(J_m) / R ** 3 + np.asarray(Jd) / (c * R ** 2), d)
+    return dV / FOURPI * E, dV / FOURPI * B
+
+
+def test_centred_derivative_newest_step_is_one_sided():
+    """Q2 / SURVEY.md 8c definition of D, end m = T-1: (f[T-1] - f[T-2])/dt -- NOT /(2 dt).
+    c dt = 1 and R = 0.08 (outside rcut = 0.05) give q = 0.08, k = 0, so evaluating the newest
+    step n = T-1 reads the record m = T-1 itself.  By hand, T = 6, dt = 0.5, c = 2:
+      rho[5] = 26, rho[4] = 17  ->  rho_dot = 9/0.5 = 18           (half-weighted: 9)
+      J[5] = (125, -50, 40), J[4] = (64, -32, 28)  ->  J_dot = (122, -36, 24)."""
+    T, dt, c = 6, 0.5, 2.0
+    rho, J = _one_cell_nonlinear(T)
+    dvec = np.array([0.048, -0.064, 0.0])                   # |d| = 0.08
+    assert oracle.lag(dvec, (0, 0, 0), dt=dt, c=c) == 0
+    E, B = oracle.fields((1, 1, 1), (0, 0, 0), (0.1, 0.1, 0.1), rho, J, dt=dt, c=c, step=T - 1,
+                         obs_xyz=[dvec], nthreads=1)
+    Ee, Be = _one_cell_expect(dvec, c, 26.0, 18.0, (125.0, -50.0, 40.0), (122.0, -36.0, 24.0))
+    np.testing.assert_allclose(E[:, 0], Ee, rtol=1e-13)
+    np.testing.assert_allclose(B[:, 0], Be, rtol=1e-13)
+
+
+def test_centred_derivative_oldest_step_is_one_sided():
+    """Q2, end m = 0: (f[1] - f[0])/dt.  Same geometry (k = 0), evaluated at n = 0.  By hand:
+      rho[0] = 1, rho[1] = 2 -> rho_dot = 1/0.5 = 2;  J[0] = 0, J[1] = (1, -2, 4) -> J_dot = (2, -4, 8)."""
+    T, dt, c = 6, 0.5, 2.0
+    rho, J = _one_cell_nonlinear(T)
+    dvec = np.array([0.048, -0.064, 0.0])
+    E, B = oracle.fields((1, 1, 1), (0, 0, 0), (0.1, 0.1, 0.1), rho, J, dt=dt, c=c, step=0,
+                         obs_xyz=[dvec], nthreads=1)
+    Ee, Be = _one_cell_expect(dvec, c, 1.0, 2.0, (0.0, 0.0, 0.0), (2.0, -4.0, 8.0))
+    np.testing.assert_allclose(E[:, 0], Ee, rtol=1e-13)
+    np.testing.assert_allclose(B[:, 0], Be, rtol=1e-13)
+
+
+def test_centred_derivative_interior_step_same_geometry():
+    """The interior formula in the same k = 0 set-up (n = 3): (f[4] - f[2])/(2 dt).  By hand:
+      rho: (17 - 5)/1 = 12;  J[3] = (27, -18, 18), J_dot = ((64-8), (-32+8), (28-10))/1 = (56, -24, 18)."""
+    T, dt, c = 6, 0.5, 2.0
+    rho, J = _one_cell_nonlinear(T)
+    dvec = np.array([0.048, -0.064, 0.0])
+    E, B = oracle.fields((1, 1, 1), (0, 0, 0), (0.1, 0.1, 0.1), rho, J, dt=dt, c=c, step=3,
+                         obs_xyz=[dvec], nthreads=1)
+    Ee, Be = _one_cell_expect(dvec, c, 10.0, 12.0, (27.0, -18.0, 18.0), (56.0, -24.0, 18.0))
+    np.testing.assert_allclose(E[:, 0], Ee, rtol=1e-13)
+    np.testing.assert_allclose(B[:, 0], Be, rtol=1e-13)
+
+
+def test_single_stored_step_has_zero_derivative():
+    """Q2, T = 1: no second snapshot exists, D = 0 in centred mode: pure Coulomb + Biot-Savart of
+    the one stored record (rho = 1, J = 0 from the recipe above is too dull: use rho = 3, J = (1,2,-1)).
+    In the paper's backward mode f[-1] = 0 gives D = f[0]/dt instead."""
+    rho = np.full((1, 1, 1, 1), 3.0)
+    J = np.array([1.0, 2.0, -1.0]).reshape(1, 3, 1, 1, 1)
+    dvec = np.array([0.0, 0.06, 0.08])                      # |d| = 0.1, q = 0.1 -> k = 0
+    kw = dict(dt=0.5, c=2.0, step=0, obs_xyz=[dvec], nthreads=1)
+    E, B = oracle.fields((1, 1, 1), (0, 0, 0), (0.1, 0.1, 0.1), rho, J, **kw)
+    Ee, Be = _one_cell_expect(dvec, 2.0, 3.0, 0.0, (1.0, 2.0, -1.0), (0.0, 0.0, 0.0))
+    np.testing.assert_allclose(E[:, 0], Ee, rtol=1e-13)
+    np.testing.assert_allclose(B[:, 0], Be, rtol=1e-13)
+    E1, B1 = oracle.fields((1, 1, 1), (0, 0, 0), (0.1, 0.1, 0.1), rho, J, deriv_mode=1, **kw)
+    Ee1, Be1 = _one_cell_expect(dvec, 2.0, 3.0, 6.0, (1.0, 2.0, -1.0), (2.0, 4.0, -2.0))
+    np.testing.assert_allclose(E1[:, 0], Ee1, rtol=1e-13)
+    np.testing.assert_allclose(B1[:, 0], Be1, rtol=1e-13)
+
+
+@pytest.mark.parametrize("R,k_expect", [(0.3125, 3), (0.0625, 1), (0.4375, 4), (0.5625, 5)])
+def test_rounding_tie_goes_up(R, k_expect):
+    """Q3: k = floor(q + 1/2) -- an exact tie rounds UP (round-half-even would give 2 at q = 2.5,
+    0 at q = 0.5 and 4 at q = 4.5).  Binary-exact numbers: c = 1, dt = 0.125, axis-aligned
+    R = 0.3125 = 2.5 dt (0.0625 = 0.5 dt, 0.4375 = 3.5 dt, 0.5625 = 4.5 dt), all representable, so
+    q is the exact half-integer in the oracle's arithmetic.  A charge switched on at step m0 in
+    backward mode is first seen at exactly n = m0 + k (no precursor), which fixes k."""
+    dt, c, T, m0, q0 = 0.125, 1.0, 16, 4, 2.0
+    dvec = np.array([R, 0.0, 0.0])
+    assert R / (c * dt) == k_expect - 0.5                   # an exact tie
+    assert oracle.lag(dvec, (0, 0, 0), dt=dt, c=c) == k_expect
+    rho = np.zeros((T, 1, 1, 1)); rho[m0:] = q0
+    J = np.zeros((T, 3, 1, 1, 1))
+    first = None
+    for n in range(T):
+        E, _ = oracle.fields((1, 1, 1), (0, 0, 0), (0.1, 0.1, 0.1), rho, J, dt=dt, c=c, step=n,
+                             obs_xyz=[dvec], deriv_mode=1, nthreads=1)
+        if first is None and E[0, 0] != 0.0:
+            first = n
+            # the switch-on spike of the backward difference, closed form
+            expect = 1e-3 / FOURPI * R * (q0 / R ** 3 + q0 / (dt * c * R ** 2))
+            assert E[0, 0] == pytest.approx(expect, rel=1e-13)
+    assert first == m0 + k_expect
