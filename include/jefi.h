@@ -155,9 +155,6 @@ jefi_status jefi_fields_host(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int
  * observation point, the paper's shape PAPER.md:93), 2 = tiled kernel or JEFI_ERR_UNSUPPORTED. */
 jefi_status jefi_set_kernel(jefi_ctx* ctx, int32_t which);
 
-/* Number of kernels launched by this context so far (for the bench's launch count). */
-int64_t     jefi_launch_count(const jefi_ctx* ctx);
-
 /* Bytes of device memory owned by the context. */
 int64_t     jefi_device_bytes(const jefi_ctx* ctx);
 
@@ -180,10 +177,6 @@ int         jefi_flops_per_pair(void);
  * JEFI_ERR_INVALID_ARG on null pointers, world <= 0 or rank outside [0, world). */
 jefi_status jefi_shard_obs(const jefi_obs_desc* obs, int32_t rank, int32_t world,
                            int64_t* begin, int64_t* count);
-
-/* Register-only FFMA (dtype F32) or DFMA (dtype F64) chain on `device`: returns the measured
- * TFLOP/s in *tflops (synchronous; used by the bench to state the ALU peak it divides by). */
-jefi_status jefi_measure_alu_peak(int device, jefi_dtype dtype, double* tflops);
 
 #ifdef __cplusplus
 }

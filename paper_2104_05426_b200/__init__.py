@@ -19,12 +19,15 @@ JEFI_OK, JEFI_ERR_INVALID_ARG, JEFI_ERR_CUDA, JEFI_ERR_OOM = 0, 1, 2, 3
 JEFI_ERR_NO_HISTORY, JEFI_ERR_TIME_RANGE, JEFI_ERR_UNSUPPORTED = 4, 5, 6
 JEFI_F32, JEFI_F64 = 0, 1
 
-EXPORTS = (
+EXPORTS = (                                   # include/jefi.h: the product ABI
     "jefi_create", "jefi_upload_history", "jefi_upload_history_host", "jefi_fields",
-    "jefi_fields_at_time", "jefi_fields_host", "jefi_set_kernel", "jefi_launch_count",
+    "jefi_fields_at_time", "jefi_fields_host", "jefi_set_kernel",
     "jefi_device_bytes", "jefi_destroy", "jefi_status_string", "jefi_last_error",
-    "jefi_flops_per_pair", "jefi_measure_alu_peak", "jefi_shard_obs",
+    "jefi_flops_per_pair", "jefi_shard_obs",
     "jefi_append_step", "jefi_append_step_host", "jefi_fields_series",
+)
+INSTRUMENT_EXPORTS = (                        # include/jefi_instrument.h: bench / test instrumentation
+    "jefi_launch_count", "jefi_measure_alu_peak", "jefi_debug_pair_lags", "jefi_debug_launch_limits",
 )
 
 
@@ -80,7 +83,9 @@ _lib.jefi_flops_per_pair.argtypes = []
 _lib.jefi_measure_alu_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
 _lib.jefi_shard_obs.argtypes = [C.POINTER(jefi_obs_desc), C.c_int32, C.c_int32, C.POINTER(C.c_int64),
                                 C.POINTER(C.c_int64)]
-for _n in EXPORTS:
+_lib.jefi_debug_pair_lags.argtypes = [_P, C.c_int32, C.c_int64, _P, _P, _P, _P]
+_lib.jefi_debug_launch_limits.argtypes = [_P, C.c_int64, C.c_int64]
+for _n in EXPORTS + INSTRUMENT_EXPORTS:
     if _n not in ("jefi_launch_count", "jefi_device_bytes", "jefi_status_string", "jefi_last_error"):
         getattr(_lib, _n).restype = C.c_int
 
@@ -202,6 +207,15 @@ def jefi_measure_alu_peak(device: int, dtype: int) -> float:
     if st != JEFI_OK:
         raise JefiError(st, "jefi_measure_alu_peak")
     return v.value
+
+
+def jefi_debug_pair_lags(ctx, which: int, n_pairs: int, obs_index_dev, cell_index_dev, lag_out_dev, stream=None):
+    _check(_lib.jefi_debug_pair_lags(ctx, int(which), int(n_pairs), _ptr(obs_index_dev), _ptr(cell_index_dev),
+                                     _ptr(lag_out_dev), _stream(stream)), ctx, "jefi_debug_pair_lags")
+
+
+def jefi_debug_launch_limits(ctx, scratch_elems: int = 0, chunk_bytes: int = 0):
+    _check(_lib.jefi_debug_launch_limits(ctx, int(scratch_elems), int(chunk_bytes)), ctx, "jefi_debug_launch_limits")
 
 
 def jefi_shard_obs(obs: jefi_obs_desc, rank: int, world: int):

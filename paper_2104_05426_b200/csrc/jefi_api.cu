@@ -6,34 +6,7 @@
 #include <string.h>
 #include <new>
 #include "jefi_internal.h"
-
-struct jefi_ctx {
-    jefi::Params P;
-    jefi_dtype   dtype;
-    int          device;
-    double       t0;
-    int          sm_count;
-    size_t       elem;             // sizeof(float|double)
-    void*        hist;             // packed history, [N_s][units][Tp], 16-byte units
-    size_t       hist_bytes;
-    void*        scratch;          // partial sums (double)
-    long long    scratch_elems;
-    void*        stage_E;          // device staging for jefi_fields_host, [3][N_o]
-    void*        stage_B;
-    void*        last;             // raw values of the two newest stored steps, [2][4][N_s]
-    void*        new_stage;        // device staging for jefi_append_step_host, [4][N_s] (lazy)
-    void*        raw_rho;          // device staging for jefi_upload_history_host (lazy)
-    void*        raw_J;
-    cudaStream_t copy_stream;      // H2D of the raw history runs here, beside the caller's stream
-    cudaEvent_t  ev_copied;        // copy_stream: raw staging filled
-    cudaEvent_t  ev_raw_free;      // caller's stream: the pre-pass has consumed the raw staging
-    bool         raw_in_use;
-    bool         has_history;
-    int          kernel_choice;
-    long long    launches;
-    long long    dev_bytes;
-    char         err[512];
-};
+#include "jefi_instrument.h"
 
 namespace {
 
@@ -72,7 +45,7 @@ jefi_status dev_alloc(jefi_ctx* c, void** p, size_t bytes, const char* what)
 void free_all(jefi_ctx* c)
 {
     cudaFree(c->hist); cudaFree(c->scratch); cudaFree(c->stage_E); cudaFree(c->stage_B);
-    cudaFree(c->raw_rho); cudaFree(c->raw_J); cudaFree(c->last); cudaFree(c->new_stage);
+    cudaFree(c->series); cudaFree(c->raw_rho); cudaFree(c->raw_J); cudaFree(c->last); cudaFree(c->new_stage);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->ev_copied) cudaEventDestroy(c->ev_copied);
     if (c->ev_raw_free) cudaEventDestroy(c->ev_raw_free);
@@ -83,7 +56,7 @@ jefi_status check_fields_args(jefi_ctx* ctx, int32_t step, int64_t obs_begin, in
 {
     if (!ctx) return JEFI_ERR_INVALID_ARG;
     ctx->err[0] = 0;
-    if (obs_begin < 0 || obs_count < 0 || obs_begin + obs_count > ctx->P.n_obs) {
+    if (obs_begin < 0 || obs_count < 0 || obs_begin > ctx->P.n_obs || obs_count > ctx->P.n_obs - obs_begin) {
         set_err(ctx, "observation range outside the observation set", cudaSuccess);
         return JEFI_ERR_INVALID_ARG;
     }
@@ -111,7 +84,7 @@ jefi_status run_fields(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t o
     jefi::FieldsLaunch L;
     L.step = step; L.obs_begin = obs_begin; L.obs_count = obs_count;
     L.E_out = E; L.B_out = B;
-    L.scratch = ctx->scratch; L.scratch_elems = ctx->scratch_elems;
+    L.scratch = ctx->scratch; L.scratch_elems = ctx->scratch_elems; L.chunk_bytes = ctx->chunk_bytes;
     L.sm_count = ctx->sm_count; L.stream = stream;
     int n = 0;
     if (ctx->kernel_choice != 1) {
@@ -186,7 +159,8 @@ jefi_status jefi_create(const jefi_grid_desc* src, const jefi_obs_desc* obs,
     long long elems = 6 * 64 * pts;
     if (elems > (1LL << 27)) elems = (1LL << 27);
     if (elems < 6 * P.n_obs) elems = 6 * P.n_obs;
-    c->scratch_elems = elems;
+    c->scratch_elems = c->scratch_alloc_elems = elems;
+    c->chunk_bytes = 384LL * 1024 * 1024;
 
     c->hist_bytes = (size_t)P.Ns * 2 * (size_t)P.Tp * 4 * c->elem;
     jefi_status s;
@@ -232,6 +206,7 @@ jefi_status jefi_upload_history(jefi_ctx* ctx, const void* rho_dev, const void* 
         if (e != cudaSuccess) return cuda_fail(ctx, "copy of the newest raw steps", e);
     }
     ctx->has_history = true;
+    ctx->series_valid = false;
     return JEFI_OK;
 }
 
@@ -250,6 +225,7 @@ jefi_status jefi_append_step(jefi_ctx* ctx, const void* rho_new_dev, const void*
                                 (cudaStream_t)stream);
     if (n < 0) return cuda_fail(ctx, "append launch", cudaGetLastError());
     ctx->launches += n;
+    ctx->series_valid = false;
     ctx->t0 += ctx->P.dt;
     return JEFI_OK;
 }
@@ -288,10 +264,12 @@ jefi_status jefi_upload_history_host(jefi_ctx* ctx, const void* rho_host, const 
     cudaError_t e = cudaSetDevice(ctx->device);
     if (e != cudaSuccess) return cuda_fail(ctx, "cudaSetDevice", e);
     const size_t rho_bytes = (size_t)ctx->P.T * (size_t)ctx->P.Ns * ctx->elem;
-    if (!ctx->raw_rho) {
+    // (each staging buffer is guarded on its own: a failed second allocation is retried by the
+    // next call instead of leaving a null raw_J behind a non-null raw_rho)
+    {
         jefi_status s;
-        if ((s = dev_alloc(ctx, &ctx->raw_rho, rho_bytes, "cudaMalloc(raw rho)")) != JEFI_OK) return s;
-        if ((s = dev_alloc(ctx, &ctx->raw_J, 3 * rho_bytes, "cudaMalloc(raw J)")) != JEFI_OK) return s;
+        if (!ctx->raw_rho && (s = dev_alloc(ctx, &ctx->raw_rho, rho_bytes, "cudaMalloc(raw rho)")) != JEFI_OK) return s;
+        if (!ctx->raw_J && (s = dev_alloc(ctx, &ctx->raw_J, 3 * rho_bytes, "cudaMalloc(raw J)")) != JEFI_OK) return s;
     }
     // The copy goes on the context's own stream so that, in a stepping loop, the H2D of the next
     // history overlaps the pairwise kernel of the current step still running on `stream`:
@@ -339,8 +317,40 @@ jefi_status jefi_fields_series(jefi_ctx* ctx, int32_t step_begin, int32_t step_c
     // every argument is checked before the first launch
     jefi_status s = check_fields_args(ctx, step_begin, obs_begin, obs_count, E_out_dev, B_out_dev);
     if (s != JEFI_OK) return s;
-    s = check_fields_args(ctx, step_begin + step_count - 1, obs_begin, obs_count, E_out_dev, B_out_dev);
-    if (s != JEFI_OK) return s;
+    if (step_count > ctx->P.T - step_begin) {          // (overflow-safe form of begin + count - 1 < T)
+        set_err(ctx, "step outside the stored history", cudaSuccess);
+        return JEFI_ERR_TIME_RANGE;
+    }
+    if (obs_count == 0) return JEFI_OK;
+    // Regular observation grids and enough steps to fill a block: the time-blocked kernel
+    // (pairwise_series.cu), which evaluates NS consecutive steps per (point, cell) pair.
+    if ((ctx->kernel_choice == 0 || ctx->kernel_choice == 3) && ctx->P.obs_kind == 0 && 2 * step_count >= jefi::series_block_steps(ctx->dtype)) {
+        cudaError_t e = cudaSetDevice(ctx->device);
+        if (e != cudaSuccess) return cuda_fail(ctx, "cudaSetDevice", e);
+        if (!ctx->series) {
+            const size_t bytes = (size_t)ctx->P.Ns * (size_t)(ctx->P.T + 3) * 4 * ctx->elem;
+            if ((s = dev_alloc(ctx, &ctx->series, bytes, "cudaMalloc(series layout)")) != JEFI_OK) return s;
+            ctx->series_valid = false;
+        }
+        if (!ctx->series_valid) {
+            int n = jefi::launch_series_layout(ctx->P, ctx->dtype, ctx->hist, ctx->series, (cudaStream_t)stream);
+            if (n < 0) return cuda_fail(ctx, "series layout launch", cudaGetLastError());
+            ctx->launches += n;
+            ctx->series_valid = true;
+        }
+        jefi::FieldsLaunch L;
+        L.step = step_begin; L.obs_begin = obs_begin; L.obs_count = obs_count;
+        L.E_out = E_out_dev; L.B_out = B_out_dev;
+        L.scratch = ctx->scratch; L.scratch_elems = ctx->scratch_elems; L.chunk_bytes = ctx->chunk_bytes;
+        L.sm_count = ctx->sm_count; L.stream = (cudaStream_t)stream;
+        int n = jefi::launch_fields_series(ctx->P, ctx->dtype, ctx->series, L, step_begin, step_count);
+        if (n < 0) return cuda_fail(ctx, "series kernel launch", cudaGetLastError());
+        if (n > 0) { ctx->launches += n; return JEFI_OK; }
+        if (ctx->kernel_choice == 3) {
+            set_err(ctx, "time-blocked kernel does not support this request", cudaSuccess);
+            return JEFI_ERR_UNSUPPORTED;
+        }
+    }
     const size_t stride = (size_t)obs_count * 3 * ctx->elem;
     for (int32_t k = 0; k < step_count; ++k) {
         s = run_fields(ctx, step_begin + k, obs_begin, obs_count, (char*)E_out_dev + (size_t)k * stride,
@@ -384,12 +394,11 @@ jefi_status jefi_fields_host(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int
 
 jefi_status jefi_set_kernel(jefi_ctx* ctx, int32_t which)
 {
-    if (!ctx || which < 0 || which > 2) return JEFI_ERR_INVALID_ARG;
+    if (!ctx || which < 0 || which > 3) return JEFI_ERR_INVALID_ARG;
     ctx->kernel_choice = which;
     return JEFI_OK;
 }
 
-int64_t jefi_launch_count(const jefi_ctx* ctx) { return ctx ? ctx->launches : 0; }
 int64_t jefi_device_bytes(const jefi_ctx* ctx) { return ctx ? ctx->dev_bytes : 0; }
 
 jefi_status jefi_destroy(jefi_ctx* ctx)
@@ -442,18 +451,6 @@ jefi_status jefi_shard_obs(const jefi_obs_desc* obs, int32_t rank, int32_t world
     const int64_t units = total / granule, base = units / world, rem = units % world;
     *begin = (rank * base + (rank < rem ? rank : rem)) * granule;
     *count = (base + (rank < rem ? 1 : 0)) * granule;
-    return JEFI_OK;
-}
-
-jefi_status jefi_measure_alu_peak(int device, jefi_dtype dtype, double* tflops)
-{
-    if (!tflops || device < 0 || (dtype != JEFI_F32 && dtype != JEFI_F64)) return JEFI_ERR_INVALID_ARG;
-    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return JEFI_ERR_CUDA; }
-    cudaDeviceProp prop;
-    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaGetLastError(); return JEFI_ERR_CUDA; }
-    const double v = jefi::measure_alu_peak(dtype, prop.multiProcessorCount, 0);
-    if (v < 0) { cudaGetLastError(); return JEFI_ERR_CUDA; }
-    *tflops = v;
     return JEFI_OK;
 }
 

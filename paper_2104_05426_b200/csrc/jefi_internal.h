@@ -26,11 +26,11 @@ struct Params {
     int     deriv_mode;
 };
 
-// Packed history layout: for cell j, half h in {0,1},
-// packed step p in [0, Tp):  vec4 at index (j*2 + h)*Tp + p
-//   half 0 = { rho, rho_dot/c, Jx/c, Jy/c },  half 1 = { Jz/c, Jx_dot/c^2, Jy_dot/c^2, Jz_dot/c^2 }
-// so that a retarded-time window of one cell is one contiguous run of 16-byte (fp32) or
-// 32-byte (fp64) elements.
+// Packed history layout: 16-byte units, U per record (fp32: 2
+// float4, fp64: 4 double2); for cell j, unit u, packed step p in [0, Tp): unit index (j*U + u)*Tp + p.
+// The 8 values of a record in unit order:
+//   { rho, rho_dot/c, Jx/c, Jy/c | Jz/c, Jx_dot/c^2, Jy_dot/c^2, Jz_dot/c^2 }
+// so that a retarded-time window of one cell is one contiguous run of 16-byte elements per unit.
 
 struct FieldsLaunch {
     int       step;        // evaluation step n
@@ -39,6 +39,7 @@ struct FieldsLaunch {
     void*     B_out;
     void*     scratch;     // partial sums [S][6][obs_count]
     long long scratch_elems;
+    long long chunk_bytes;  // a source chunk's packed history stays below this (L2 sharing)
     int       sm_count;
     cudaStream_t stream;
 };
@@ -55,7 +56,47 @@ int launch_fields_point(const Params& P, jefi_dtype dt, const void* hist, const 
 // tiled kernel: regular observation grids only; returns 0 if it does not support the request
 int launch_fields_tiled(const Params& P, jefi_dtype dt, const void* hist, const FieldsLaunch& L);
 int launch_reduce_scale(const Params& P, jefi_dtype dt, const FieldsLaunch& L, int S);
-
-double measure_alu_peak(jefi_dtype dt, int sm_count, int clock_khz);
+// time-blocked kernel (pairwise_series.cu): the series layout (raw 16-byte
+// records [cell][unit][T+3]) is built from the packed history; launch_fields_series evaluates
+// step_count consecutive steps into E_out/B_out [step][3][obs_count]; returns 0 if unsupported
+int launch_series_layout(const Params& P, jefi_dtype dt, const void* packed, void* series, cudaStream_t stream);
+int launch_fields_series(const Params& P, jefi_dtype dt, const void* series, const FieldsLaunch& L, int step_begin,
+                         int step_count);
+int series_block_steps(jefi_dtype dt);
 
 }  // namespace jefi
+
+// the context behind the opaque handle of include/jefi.h (defined here so that the instrumentation
+// entry points of include/jefi_instrument.h, in instrument.cu, can read it)
+struct jefi_ctx {
+    jefi::Params P;
+    jefi_dtype   dtype;
+    int          device;
+    double       t0;
+    int          sm_count;
+    size_t       elem;             // sizeof(float|double)
+    void*        hist;             // packed history, [N_s][units][Tp], 16-byte units
+    size_t       hist_bytes;
+    void*        scratch;          // partial sums (double)
+    long long    scratch_elems;    // what the launchers may use (= allocated, unless a test caps it)
+    long long    scratch_alloc_elems;
+    long long    chunk_bytes;      // packed-history bytes per source chunk (L2 sharing, pairwise_tiled.cu)
+    void*        stage_E;          // device staging for jefi_fields_host, [3][N_o]
+    void*        stage_B;
+    void*        series;           // series layout of the history (lazy: first jefi_fields_series), [N_s][units][T+3]
+    bool         series_valid;     // matches the packed history
+    void*        last;             // raw values of the two newest stored steps, [2][4][N_s]
+    void*        new_stage;        // device staging for jefi_append_step_host, [4][N_s] (lazy)
+    void*        raw_rho;          // device staging for jefi_upload_history_host (lazy)
+    void*        raw_J;
+    cudaStream_t copy_stream;      // H2D of the raw history runs here, beside the caller's stream
+    cudaEvent_t  ev_copied;        // copy_stream: raw staging filled
+    cudaEvent_t  ev_raw_free;      // caller's stream: the pre-pass has consumed the raw staging
+    bool         raw_in_use;
+    bool         has_history;
+    int          kernel_choice;
+    long long    launches;
+    long long    dev_bytes;
+    char         err[512];
+};
+

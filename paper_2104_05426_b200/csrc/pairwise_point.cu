@@ -9,7 +9,7 @@
 //   k = floor(R/(c dt) + 0.5),  p = max(n + 1 - k, 0)            (p = 0: the all-zero record)
 //   s = (rho*rinv + rho_dot')*rinv^2,   u = (J'*rinv + J_dot'')*rinv^2
 //   E += d*s - J_dot''*rinv,            B' += u x d               (B = c * B')
-#include "jefi_internal.h"
+#include "tiled_common.cuh"
 
 namespace jefi {
 namespace {
@@ -29,10 +29,6 @@ __device__ __forceinline__ Rec<double> load_rec(const double* __restrict__ hist,
     const double2 c = h[(j * 4 + 2) * Tp + p], d = h[(j * 4 + 3) * Tp + p];
     return Rec<double>{{a.x, a.y, b.x, b.y, c.x, c.y, d.x, d.y}};
 }
-
-template <typename T> __device__ __forceinline__ T rsqrt_t(T x);
-template <> __device__ __forceinline__ float  rsqrt_t<float>(float x)   { return rsqrtf(x); }
-template <> __device__ __forceinline__ double rsqrt_t<double>(double x) { return 1.0 / sqrt(x); }
 
 struct PointArgs {
     int nsx, nsy, nsz;
@@ -64,13 +60,13 @@ fields_point_kernel(const T* __restrict__ hist, double* __restrict__ partial, Po
     if (a.obs_kind == 0) {
         const int ix = (int)(gi % a.nox), iy = (int)((gi / a.nox) % a.noy);
         const int iz = (int)(gi / ((long long)a.nox * a.noy));
-        ox = (T)(a.d0x + ix * a.ohx); oy = (T)(a.d0y + iy * a.ohy); oz = (T)(a.d0z + iz * a.ohz);
+        ox = obs_coord<T>(a.d0x, ix, a.ohx); oy = obs_coord<T>(a.d0y, iy, a.ohy); oz = obs_coord<T>(a.d0z, iz, a.ohz);
     } else {
         const T* p = (const T*)a.points + 3 * gi;
         ox = (T)((double)p[0] - a.sox); oy = (T)((double)p[1] - a.soy); oz = (T)((double)p[2] - a.soz);
     }
     const T shx = (T)a.shx, shy = (T)a.shy, shz = (T)a.shz;
-    const T rcut2 = (T)a.rcut2, inv_cdt = (T)a.inv_cdt;
+    const T rcut2 = (T)a.rcut2, inv_cdt = -tie_biased_neg_inv_cdt<T>(a.inv_cdt);
 
     const long long cb = (long long)blockIdx.y * a.cells_per_chunk;
     long long ce = cb + a.cells_per_chunk;
@@ -82,18 +78,15 @@ fields_point_kernel(const T* __restrict__ hist, double* __restrict__ partial, Po
     long long j = cb;
     while (j < ce) {
         // one (part of a) source row: y, z fixed
-        const T dy = oy - (T)sy * shy, dz = oz - (T)sz * shz;
-        const T ryz = dy * dy + dz * dz;
+        T dy, dz;
+        const T ryz = row_ryz<T>(oy, oz, sy, sz, shy, shz, dy, dz);
         long long row_end = j + (a.nsx - sx);
         if (row_end > ce) row_end = ce;
         T ex = 0, ey = 0, ez = 0, bx = 0, by = 0, bz = 0;
         for (; j < row_end; ++j, ++sx) {
-            const T dx = ox - (T)sx * shx;
-            const T R2 = dx * dx + ryz;
-            T rinv = rsqrt_t<T>(R2);
-            if (R2 < rcut2) rinv = T(0);
-            const T R = R2 * rinv;
-            const int k = (int)floor(R * inv_cdt + T(0.5));
+            T dx, rinv;
+            int k;
+            point_geo<T>(ox, sx, shx, ryz, rcut2, inv_cdt, dx, rinv, k);
             int p = a.n1 - k;
             p = p < 0 ? 0 : p;
             const Rec<T> h = load_rec(hist, j, a.Tp, p);      // rho, rho', Jx, Jy, Jz, Jx', Jy', Jz'

@@ -12,9 +12,12 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
 
 
-def rel_l2(got, ref, field_ref=None, tol=None):
+def rel_l2(got, ref, field_ref=None, tol=None, comp_floor=1e-12):
     """Per-component relative L2 error with the zero-component rule (Q10):
-    if ||ref_c|| < 1e-12 * ||ref field|| the error is measured against the whole field's norm."""
+    if ||ref_c|| < comp_floor * ||ref field|| (1e-12: an identically-zero component) the error is
+    measured against the whole field's norm.  The fp32 fuzz over few-point observation sets
+    passes comp_floor = 1e-3: with two or three points a component can cancel to 1e-5 of the
+    field by chance, and no fp32 sum of O(field) terms resolves that to 2e-4 of ITSELF."""
     import numpy as np
 
     got = np.asarray(got, dtype=np.float64)
@@ -23,6 +26,6 @@ def rel_l2(got, ref, field_ref=None, tol=None):
     out = []
     for c in range(ref.shape[0]):
         rn = float(np.linalg.norm(ref[c]))
-        den = rn if rn >= 1e-12 * fnorm and rn > 0 else (fnorm if fnorm > 0 else 1.0)
+        den = rn if rn >= comp_floor * fnorm and rn > 0 else (fnorm if fnorm > 0 else 1.0)
         out.append(float(np.linalg.norm(got[c] - ref[c])) / den)
     return out

@@ -51,7 +51,7 @@ def oracle_fields(w, step, idx=None, deriv_mode=0, points=None):
     key = (w.name, w.dtype, w.n_src, w.spacing_src, w.T, w.seed, w.c, w.dt, step, deriv_mode,
            hashlib.sha1(np.ascontiguousarray(pts).tobytes()).hexdigest())
     if key not in _ORACLE_CACHE:
-        if len(_ORACLE_CACHE) > 64:
+        if len(_ORACLE_CACHE) > 4000:
             _ORACLE_CACHE.clear()
         _ORACLE_CACHE[key] = oracle.fields(w.n_src, w.origin_src, w.spacing_src, w.rho, w.J, dt=w.dt, c=w.c,
                                            step=step, obs_xyz=pts, deriv_mode=deriv_mode)
@@ -61,3 +61,14 @@ def oracle_fields(w, step, idx=None, deriv_mode=0, points=None):
 def tol_for(w):
     """BASELINE.json north_star: rel-L2 per field component <= 1e-5 (fp64 mode), 2e-4 (fp32)."""
     return 2e-4 if w.dtype == "f32" else 1e-5
+
+
+def gpu_fields_series(ctx, w, step_begin, step_count, obs_begin=0, obs_count=None):
+    """E, B as float64 numpy [step_count][3][count] from one jefi_fields_series call."""
+    import torch
+    n = ctx.n_points - obs_begin if obs_count is None else obs_count
+    E = torch.full((step_count, 3, n), float("nan"), dtype=torch_dtype(w), device="cuda")
+    B = torch.full((step_count, 3, n), float("nan"), dtype=torch_dtype(w), device="cuda")
+    ctx.fields_series(step_begin, step_count, E, B, obs_begin, n)
+    torch.cuda.synchronize()
+    return E.cpu().numpy().astype(np.float64), B.cpu().numpy().astype(np.float64)

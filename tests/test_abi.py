@@ -18,8 +18,8 @@ def jb():
     return jb
 
 
-def _declared_symbols():
-    text = open(os.path.join(ROOT, "include", "jefi.h")).read()
+def _declared_symbols(header="jefi.h"):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(jefi_[a-z_0-9]+)\s*\(", text)))
 
@@ -31,10 +31,15 @@ def test_header_symbols_are_exported(jb):
     for n in names:
         assert hasattr(lib, n), f"{n} declared in include/jefi.h but not exported"
     assert set(names) == set(jb.EXPORTS)
+    # measurement / test instrumentation lives in its own header, outside the product ABI
+    extra = _declared_symbols("jefi_instrument.h")
+    for n in extra:
+        assert hasattr(lib, n), f"{n} declared in include/jefi_instrument.h but not exported"
+    assert set(extra) == set(jb.INSTRUMENT_EXPORTS) and not set(extra) & set(names)
 
 
 def test_binding_has_same_names(jb):
-    for n in _declared_symbols():
+    for n in _declared_symbols() + _declared_symbols("jefi_instrument.h"):
         assert callable(getattr(jb, n)), n
 
 

@@ -22,11 +22,23 @@ def jb():
     return jb
 
 
-def check(w, E, B, Eo, Bo, tol=None, what=""):
+POINTWISE = 20.0        # max |got - oracle| <= POINTWISE * tol * rms(oracle field); DESIGN.md section 7
+
+
+def check(w, E, B, Eo, Bo, tol=None, what="", comp_floor=1e-12):
+    """north_star's bar (rel-L2 per component) AND a bound on every single output against the
+    ORACLE: no point may be off by more than 20 tol x the rms magnitude of the reference field
+    (a norm alone lets one badly wrong output hide among 10^5 good ones)."""
     tol = tol_for(w) if tol is None else tol
     assert np.isfinite(E).all() and np.isfinite(B).all(), what
-    eE, eB = rel_l2(E, Eo, field_ref=Eo), rel_l2(B, Bo, field_ref=Bo)
+    eE = rel_l2(E, Eo, field_ref=Eo, comp_floor=comp_floor)
+    eB = rel_l2(B, Bo, field_ref=Bo, comp_floor=comp_floor)
     assert max(eE) <= tol and max(eB) <= tol, f"{what}: rel-L2 E {eE} B {eB} tol {tol}"
+    for got, ref, name in ((E, Eo, "E"), (B, Bo, "B")):
+        rms = float(np.sqrt(np.mean(np.sum(ref * ref, axis=0)))) if ref.size else 0.0
+        worst = float(np.abs(got - ref).max()) if ref.size else 0.0
+        assert worst <= POINTWISE * tol * rms, \
+            f"{what}: worst pointwise {name} error {worst:.3e} > {POINTWISE} x {tol} x rms {rms:.3e}"
     return eE, eB
 
 
@@ -83,24 +95,48 @@ def test_config2c_white_noise_history(jb, kernel, dtype):
 def test_config3_collision_full_size_sampled(jb, kernel):
     w = wl.config3_collision()
     assert w.T == 221 and w.N_s == 64 ** 3
-    run_case(jb, w, w.obs_subset(1024), kernel)
+    run_case(jb, w, w.obs_subset(16384), kernel)        # 16 384 seeded points, 4.3e9 pairs
 
 
 # ------------------------------------------------------------------ config 4
+_C4_PLAN = {}
+
+
+def c4_oracle_plan(w):
+    """SURVEY.md 8(d) coverage of config 4: the oracle on EVERY point at four of the 128 output
+    steps (first, last, two seeded) and on a seeded subset at each of the other 124.  The subset
+    is 4096 points when the host is fast enough, else as many (>= 512) as keep those 124 oracle
+    runs within ~2.5 minutes of the GPU suite's budget -- sized from the measured speed of the
+    first full step, so a slower box shrinks the sample instead of timing the suite out."""
+    import time
+    if "plan" in _C4_PLAN:                       # one plan per session: the series test reuses the oracle runs
+        return _C4_PLAN["plan"]
+    u = wl.uniform01(w.seed + 404, 0, 2)
+    inner = sorted({w.steps[1 + int(u[0] * 62)], w.steps[64 + int(u[1] * 62)]})
+    full = [w.steps[0], *inner, w.steps[-1]]
+    t0 = time.perf_counter()
+    oracle_fields(w, full[0], None)
+    rate = w.N_o * w.N_s / max(time.perf_counter() - t0, 1e-3)
+    n_sub = int(min(4096, max(512, 150.0 * rate / (124 * w.N_s))))
+    _C4_PLAN["plan"] = (full, w.obs_subset(n_sub))
+    return _C4_PLAN["plan"]
+
+
 def test_config4_detached_plane_time_series(jb):
     w = wl.config4_detached()
     assert w.T == 622 and w.steps[0] == 494 and len(w.steps) == 128
-    idx = w.obs_subset(1536)
+    full, idx = c4_oracle_plan(w)
     ctx = make_ctx(w, jb)
     try:
         upload(ctx, w)
-        checked = {w.steps[0], w.steps[-1], w.steps[37]}
         for n in w.steps:
             E, B = gpu_fields(ctx, w, n)
-            assert np.isfinite(E).all() and np.isfinite(B).all()
-            if n in checked:
+            if n in full:
+                Eo, Bo = oracle_fields(w, n, None)
+                check(w, E, B, Eo, Bo, None, f"c4 step {n} (every point)")
+            else:
                 Eo, Bo = oracle_fields(w, n, idx)
-                check(w, E[:, idx], B[:, idx], Eo, Bo, None, f"c4 step {n}")
+                check(w, E[:, idx], B[:, idx], Eo, Bo, None, f"c4 step {n} ({len(idx)} points)")
     finally:
         ctx.close()
 
@@ -109,24 +145,17 @@ def test_config4_detached_plane_time_series(jb):
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 def test_config5_large_sampled(jb, dtype):
     """100^3 x 100^3 with a history shorter than the longest delay (k_max = 343 > T-1 = 199):
-    the m < 0 rule (Q4) is live.  fp32: the whole grid; fp64: a 100x100x12 slab of it."""
+    the m < 0 rule (Q4) is live.  Both precisions evaluate the WHOLE grid on the GPU; the oracle
+    covers 8192 seeded points per precision, run on that precision's inputs."""
     w = wl.config5_large(dtype=dtype)
     ctx = make_ctx(w, jb)
     try:
         upload(ctx, w)
         n = w.steps[0]
-        if dtype == "f32":
-            begin, count = 0, w.N_o
-        else:
-            begin, count = 100 * 100 * 44, 100 * 100 * 12
-        E, B = gpu_fields(ctx, w, n, begin, count)
-        idx = w.obs_subset(400, seed_offset=1)
-        idx = idx[(idx >= begin) & (idx < begin + count)]
-        if dtype == "f64":
-            extra = begin + np.arange(0, count, 997)
-            idx = np.unique(np.concatenate([idx, extra]))[:320]
+        E, B = gpu_fields(ctx, w, n)
+        idx = w.obs_subset(8192, seed_offset=1)
         Eo, Bo = oracle_fields(w, n, idx)
-        check(w, E[:, idx - begin], B[:, idx - begin], Eo, Bo, None, f"c5 {dtype}")
+        check(w, E[:, idx], B[:, idx], Eo, Bo, None, f"c5 {dtype}")
     finally:
         ctx.close()
 
@@ -442,10 +471,11 @@ def test_paper_constant_sources_410_snapshots(jb):
         wall = time.perf_counter() - t0
         E1 = torch.empty((3, w.N_o), dtype=torch.float32, device="cuda")
         B1 = torch.empty_like(E1)
-        for n in (0, 77, 410):                             # the series equals the single calls
+        for n in (0, 77, 410):                             # the series (time-blocked kernel) vs single calls
             ctx.fields(n, E1, B1)
             torch.cuda.synchronize()
-            assert torch.equal(E1, E[n]) and torch.equal(B1, B[n])
+            assert torch.allclose(E1, E[n], rtol=0, atol=2e-5 * float(E1.abs().max()))
+            assert torch.allclose(B1, B[n], rtol=0, atol=2e-5 * float(B1.abs().max()))
         with pytest.raises(jb.JefiError) as e:
             ctx.fields_series(400, 20, E, B)
         assert e.value.status == jb.JEFI_ERR_TIME_RANGE
@@ -545,3 +575,214 @@ def test_fuzz_random_lattices_fp32(jb):
             ran += 1
         finally:
             ctx.close()
+
+
+# ------------------------------------------------------------------ retarded-index parity report
+def _kernel_lags(jb, ctx, which, obs_idx, cell_idx):
+    import torch
+    o = torch.as_tensor(np.ascontiguousarray(obs_idx, dtype=np.int64)).cuda()
+    c = torch.as_tensor(np.ascontiguousarray(cell_idx, dtype=np.int64)).cuda()
+    out = torch.full((len(obs_idx),), -7, dtype=torch.int32, device="cuda")
+    jb.jefi_debug_pair_lags(ctx.ctx, which, len(obs_idx), o, c, out)
+    torch.cuda.synchronize()
+    return out.cpu().numpy().astype(np.int64)
+
+
+def _oracle_lags(w, obs_idx, cell_idx):
+    import oracle
+    pts = w.obs_points(obs_idx)
+    nx, ny, nz = w.n_src
+    cell_idx = np.asarray(cell_idx, dtype=np.int64)
+    src = np.stack([w.origin_src[0] + (cell_idx % nx) * w.spacing_src[0],
+                    w.origin_src[1] + ((cell_idx // nx) % ny) * w.spacing_src[1],
+                    w.origin_src[2] + (cell_idx // (nx * ny)) * w.spacing_src[2]], axis=1)
+    return np.array([oracle.lag(p, s, dt=w.dt, c=w.c) for p, s in zip(pts, src)], dtype=np.int64)
+
+
+def _geometry(name, dtype):
+    """Descriptors of a config without its multi-GB history (the lag does not read it)."""
+    import test_workload_lattices as tl
+    w = tl._geometry_only(name)
+    w.dtype = dtype
+    return w
+
+
+def _sample_pairs(w, n, seed):
+    """Seeded (obs, cell) pairs: uniform over all pairs, plus -- because the near field carries the
+    largest weights -- every obs point of a seeded subset paired with its 27 nearest source cells."""
+    u = wl.uniform01(seed, 0, 2 * n)
+    obs = np.minimum((u[:n] * w.N_o).astype(np.int64), w.N_o - 1)
+    cell = np.minimum((u[n:] * w.N_s).astype(np.int64), w.N_s - 1)
+    sub = w.obs_subset(256, seed_offset=5)
+    p = w.obs_points(sub)
+    near_o, near_c = [], []
+    nx, ny, nz = w.n_src
+    base = [np.clip(np.rint((p[:, a] - w.origin_src[a]) / w.spacing_src[a]).astype(np.int64), 0, w.n_src[a] - 1)
+            for a in range(3)]
+    for dz in (-1, 0, 1):
+        for dy in (-1, 0, 1):
+            for dx in (-1, 0, 1):
+                jx, jy, jz = (np.clip(base[0] + dx, 0, nx - 1), np.clip(base[1] + dy, 0, ny - 1),
+                              np.clip(base[2] + dz, 0, nz - 1))
+                near_o.append(sub); near_c.append((jz * ny + jy) * nx + jx)
+    return np.concatenate([obs, *near_o]), np.concatenate([cell, *near_c])
+
+
+@pytest.mark.parametrize("name,dtype", [("c1", "f64"), ("c2", "f64"), ("c2", "f32"), ("c3", "f32"), ("c4", "f32"),
+                                        ("c5", "f32"), ("c5", "f64")])
+def test_retarded_index_mismatch_count_is_zero_on_every_config(jb, name, dtype):
+    """SURVEY.md 8(d) parity report: the retarded lag k the kernels compute -- dumped by
+    jefi_debug_pair_lags, which runs the very device function the pairwise kernels inline
+    (rsqrt.approx, R = R2 rinv, biased magic-constant FMA; and the per-point kernel's
+    floor(R/(c dt) + 1/2)) -- against the oracle's fp64 k on 60 000 seeded pairs plus the 27 nearest
+    cells of 256 points, on the lattice of each BASELINE.json config and precision: 0 mismatches."""
+    w = _geometry(name, dtype)
+    ctx = make_ctx(w, jb)
+    try:
+        obs, cell = _sample_pairs(w, 60000, seed=w.seed + 31)
+        ko = _oracle_lags(w, obs, cell)
+        for which in (1, 2):
+            kg = _kernel_lags(jb, ctx, which, obs, cell)
+            bad = np.nonzero(kg != ko)[0]
+            assert bad.size == 0, (f"{name} {dtype} kernel {which}: {bad.size} of {len(ko)} lags differ, e.g. pair "
+                                   f"(obs {obs[bad[0]]}, cell {cell[bad[0]]}): kernel {kg[bad[0]]} oracle {ko[bad[0]]}")
+    finally:
+        ctx.close()
+
+
+# ------------------------------------------------------------------ exact rounding ties (Q3)
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("case", ["shared_grid_cdt_2dx", "staggered_x_ratio1", "staggered_x_ratio3"])
+def test_exact_ties_on_binary_exact_lattices_round_up_like_the_oracle(jb, dtype, case):
+    """Lattices on which q = R/(c dt) is an exact half-integer for whole families of pairs AND every
+    coordinate is exact in binary (dx = 1/8), so the tie exists in the kernels' arithmetic as it
+    does in the oracle's: (a) obs = source grid with c dt = 2 dx (on-axis R = dx, 3dx, 5dx -> q =
+    0.5, 1.5, 2.5); (b), (c) obs staggered by half a cell on x only with dx/(c dt) = 1 and 3 -- the
+    Yee-style class (on-axis q = i + 1/2, 3i + 3/2; the nearest cells sit exactly ON the screening
+    radius R = dx/2, which the strict '<' of Q5 keeps).  White-noise history: one flipped index is an
+    O(1) error in its term, and the on-axis pairs are the nearest, heaviest ones.  Every kernel must
+    round these ties UP like the oracle's floor(q + 1/2): lag dump identical, fields within tolerance."""
+    dx = 0.125
+    n = (6, 5, 4)
+    org = tuple(-(a - 1) / 2 * dx for a in n)
+    if case == "shared_grid_cdt_2dx":
+        dt, origin_obs = 2 * dx, org
+    else:
+        dt = dx if case.endswith("ratio1") else dx / 3
+        origin_obs = (org[0] + dx / 2, org[1], org[2])
+    w = wl.random_history(n, 40, seed=61, dtype=dtype, spacing=(dx,) * 3, n_obs=n, origin_obs=origin_obs, dt=dt)
+    ctx = make_ctx(w, jb)
+    try:
+        obs = np.repeat(np.arange(w.N_o), w.N_s)
+        cell = np.tile(np.arange(w.N_s), w.N_o)
+        ko = _oracle_lags(w, obs, cell)
+        pts, nx, ny = w.obs_points(obs), n[0], n[1]
+        src = np.stack([w.origin_src[0] + (cell % nx) * dx, w.origin_src[1] + ((cell // nx) % ny) * dx,
+                        w.origin_src[2] + (cell // (nx * ny)) * dx], axis=1)
+        q = np.linalg.norm(pts - src, axis=1) / dt
+        ties = int(np.sum(q - np.floor(q) == 0.5))
+        assert ties >= 50, ties
+        for which in (1, 2):
+            kg = _kernel_lags(jb, ctx, which, obs, cell)
+            assert np.array_equal(kg, ko), f"{case} {dtype} kernel {which}: {int((kg != ko).sum())} lags differ"
+        upload(ctx, w)
+        for kernel in (1, 2):
+            ctx.set_kernel(kernel)
+            for step in (39, 7):
+                E, B = gpu_fields(ctx, w, step)
+                Eo, Bo = oracle_fields(w, step)
+                check(w, E, B, Eo, Bo, None, f"{case} {dtype} kernel {kernel} step {step}")
+    finally:
+        ctx.close()
+
+
+def test_ties_on_a_decimal_staggered_lattice_are_reported(jb):
+    """The same Yee-style class with DECIMAL spacing (dx = 0.1, c dt = 0.1, obs staggered by dx/2 on
+    x; dz = 0.05 keeps every pair off the screening radius, so only the tie question is left):
+    0.1 and 0.05 are not binary fractions, the on-axis q = i + 1/2 exist only up to rounding noise,
+    and which side of the tie a pair falls on is decided by the last bit -- differently in the
+    oracle's fp64, the per-point kernel's and the tiled kernel's arithmetic.  This cannot be
+    'fixed' (Q3, stated limitation); what must hold, and is asserted: (1) every pair
+    whose q is NOT within 1e-5 of a half-integer gets the oracle's lag from both kernels; (2) a
+    tie pair is off by at most one step; (3) with a history constant in time (the retarded step
+    does not matter) both kernels stay within tolerance; (4) for a smooth history the error is
+    bounded by the tie pairs' share -- measured and printed, asserted < 5 %."""
+    dx, dt = 0.1, 0.1
+    n = (6, 5, 4)
+    sp = (dx, dx, 0.05)
+    org = tuple(-(a - 1) / 2 * h for a, h in zip(n, sp))
+    w = wl.random_history(n, 40, seed=63, dtype="f32", spacing=sp, n_obs=n, spacing_obs=sp,
+                          origin_obs=(org[0] + dx / 2, org[1], org[2]), dt=dt)
+    obs = np.repeat(np.arange(w.N_o), w.N_s)
+    cell = np.tile(np.arange(w.N_s), w.N_o)
+    ko = _oracle_lags(w, obs, cell)
+    pts, nx, ny = w.obs_points(obs), n[0], n[1]
+    src = np.stack([w.origin_src[0] + (cell % nx) * sp[0], w.origin_src[1] + ((cell // nx) % ny) * sp[1],
+                    w.origin_src[2] + (cell // (nx * ny)) * sp[2]], axis=1)
+    q = np.linalg.norm(pts - src, axis=1) / dt
+    near_tie = np.abs(q - np.floor(q) - 0.5) < 1e-5
+    assert near_tie.sum() >= 100
+    ctx = make_ctx(w, jb)
+    try:
+        report = {}
+        for which in (1, 2):
+            kg = _kernel_lags(jb, ctx, which, obs, cell)
+            diff = kg != ko
+            assert not np.any(diff & ~near_tie), f"kernel {which}: a non-tie pair got a different lag"
+            assert np.abs(kg - ko).max() <= 1
+            report[which] = int(diff.sum())
+        # (3) constant-in-time history: the retarded step cannot matter
+        w.rho[:] = w.rho[0]; w.J[:] = w.J[0]
+        upload(ctx, w)
+        for kernel in (1, 2):
+            ctx.set_kernel(kernel)
+            E, B = gpu_fields(ctx, w, 39)
+            Eo, Bo = oracle_fields(w, 39)
+            check(w, E, B, Eo, Bo, None, f"decimal ties, constant history, kernel {kernel}")
+        # (4) smooth history: f(t) = f0 * (1 + 0.2 sin(2 pi m / 40))
+        mod = (1.0 + 0.2 * np.sin(2 * np.pi * np.arange(40) / 40.0)).astype(w.np_dtype)
+        w.name = "decimal_ties_smooth"
+        w.rho = np.ascontiguousarray(w.rho * mod[:, None, None, None])
+        w.J = np.ascontiguousarray(w.J * mod[:, None, None, None, None])
+        upload(ctx, w)
+        worst = 0.0
+        for kernel in (1, 2):
+            ctx.set_kernel(kernel)
+            E, B = gpu_fields(ctx, w, 39)
+            Eo, Bo = oracle_fields(w, 39)
+            worst = max(worst, max(rel_l2(E, Eo, field_ref=Eo)), max(rel_l2(B, Bo, field_ref=Bo)))
+        print(f"\ndecimal staggered lattice: {int(near_tie.sum())} tie pairs of {len(q)}; lags differing from the "
+              f"oracle: per-point kernel {report[1]}, tiled kernel {report[2]}; smooth-history rel-L2 {worst:.2e}")
+        assert worst < 5e-2
+    finally:
+        ctx.close()
+
+
+# ------------------------------------------------------------------ accumulating launches (very large histories)
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_source_chunks_spread_over_accumulating_launches(jb, dtype):
+    """When a source chunk's packed history is capped (L2 sharing) and the partial-sum scratch
+    holds fewer chunks than that needs, the launcher spreads the chunks over several launches
+    that accumulate into the same partial sums (the path of the paper's 160^3 x 500-step case).
+    Forced here on a small problem through the instrumentation hook: scratch for 3 chunks,
+    chunks of <= 48 KB of history -> 8+ chunks, 3+ launches with a short last one."""
+    w = wl.random_history((12, 10, 9), 60, seed=71, dtype=dtype, n_obs=(9, 8, 10), dt=0.05)
+    ctx = make_ctx(w, jb)
+    try:
+        upload(ctx, w)
+        ctx.set_kernel(2)
+        E0, B0 = gpu_fields(ctx, w, 59)
+        l0 = ctx.launches
+        E0, B0 = gpu_fields(ctx, w, 59)
+        single = ctx.launches - l0
+        jb.jefi_debug_launch_limits(ctx.ctx, 3 * 6 * w.N_o, 48 * 1024)
+        l0 = ctx.launches
+        E, B = gpu_fields(ctx, w, 59)
+        assert ctx.launches - l0 >= single + 2
+        Eo, Bo = oracle_fields(w, 59)
+        check(w, E, B, Eo, Bo, None, f"accumulating launches {dtype}")
+        check(w, E0, B0, Eo, Bo, None, f"single launch {dtype}")
+        E1, B1 = gpu_fields(ctx, w, 59, 100, 333)               # a sub-range through the same path
+        np.testing.assert_allclose(E1, E[:, 100:433], rtol=1e-4, atol=1e-5 * np.abs(E).max())
+    finally:
+        ctx.close()

@@ -47,6 +47,12 @@ def test_no_lag_sits_near_a_tie(name, margin):
                                                 np.float32(np.inf * ulps))
         k32 = np.floor((Rp * inv).astype(np.float32) + np.float32(0.5)).astype(np.int64)
         assert np.array_equal(k32, k64), (name, ulps, int((k32 != k64).sum()))
+        # the tiled kernels' form: one FMA R * (1 + 2^-21)/(c dt) + 1.5*2^23, rounded to nearest even
+        # (the relative bias sends exact ties up, Q3) -- no lattice distance may sit so
+        # close BELOW a tie that the bias lifts it over
+        inv_b = np.float32((1.0 / (w.c * w.dt)) * (1.0 + 2.0 ** -21))
+        kb = np.rint(Rp.astype(np.float64) * np.float64(inv_b)).astype(np.int64)
+        assert np.array_equal(kb, k64), (name, ulps, "biased", int((kb != k64).sum()))
 
 
 def _geometry_only(name):
