@@ -57,7 +57,10 @@ typedef struct {
 
 /* Observation set.  kind 0: the regular grid `grid` (the paper's case).  kind 1: an explicit
  * list of `npoints` positions, points_dev[npoints][3] of the context dtype, device memory
- * owned by the caller and read at every jefi_fields call. */
+ * owned by the caller.  The positions belong to the context as a grid does: jefi_create reads
+ * them (it sorts the points into spatially compact tiles for the tiled kernel) and every
+ * jefi_fields call reads them again; they must stay allocated and UNCHANGED until jefi_destroy.
+ * Non-finite positions are JEFI_ERR_INVALID_ARG.  Outputs are always in the caller's order. */
 typedef struct {
     int32_t        kind;
     jefi_grid_desc grid;
@@ -81,7 +84,9 @@ typedef struct {
  * ever need on it: the packed history (32 bytes (fp32) / 64 bytes (fp64) per (cell, step), plus
  * one all-zero step standing for m < 0), the raw values of the two newest steps (for
  * jefi_append_step), partial-sum scratch, and the device output staging used by
- * jefi_fields_host.  No kernel is launched.  *out is written only on success.  Synchronous. */
+ * jefi_fields_host.  For a regular observation grid no kernel is launched; for a point list
+ * (kind 1) the tiling kernels run on the default stream and are waited for.  *out is written
+ * only on success.  Synchronous. */
 jefi_status jefi_create(const jefi_grid_desc* src, const jefi_obs_desc* obs,
                         const jefi_time_desc* time, jefi_dtype dtype, int device,
                         jefi_ctx** out);
@@ -131,13 +136,30 @@ jefi_status jefi_fields(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t 
                         void* E_out_dev, void* B_out_dev, jefi_stream stream);
 
 /* A time series in one call (the paper evaluates hundreds of snapshots on fixed grids,
- * PAPER.md:213-219; BASELINE.json configs[3] asks for 128 output steps): the same as
- * step_count calls of jefi_fields for step_begin, step_begin+1, ... with outputs
- * E_out_dev[step_count][3][obs_count], B_out_dev likewise.  All launches are enqueued on
- * `stream` back to back; step_count = 0 is a no-op. */
+ * PAPER.md:213-219; BASELINE.json configs[3] asks for 128 output steps): the fields of
+ * step_begin, step_begin+1, ... as step_count calls of jefi_fields would give them (same
+ * definition, same tolerances; not the same bits), outputs E_out_dev[step_count][3][obs_count],
+ * B_out_dev likewise.  On regular observation grids with at least half a block of steps
+ * (block = 6 steps in fp32, 4 in fp64) this runs the time-blocked kernel:
+ * the geometry and the retarded lag of a (point, cell) pair do not depend on the evaluation
+ * step (Eq. (6)), so a thread computes them once and walks a block of consecutive
+ * output steps, whose retarded steps are consecutive stored snapshots; it reads a second copy
+ * of the history ("series layout": the raw 16-byte {rho, J/c} record per (cell, step), time
+ * differences formed in registers), which the context allocates on the first such call
+ * (N_s x (nsteps+3) x 16 B (fp32) / 32 B (fp64)) and rebuilds from the packed history after
+ * every jefi_upload_history / jefi_append_step.  Other requests (point lists, one or two steps,
+ * windows beyond shared memory) run step_count one-step evaluations.  All launches are enqueued
+ * on `stream` back to back; step_count = 0 is a no-op. */
 jefi_status jefi_fields_series(jefi_ctx* ctx, int32_t step_begin, int32_t step_count,
                                int64_t obs_begin, int64_t obs_count,
                                void* E_out_dev, void* B_out_dev, jefi_stream stream);
+
+/* Same, results copied to HOST buffers [step_count][3][obs_count] on `stream` through a device
+ * staging area owned by the context (allocated on first use, grown when a larger series is
+ * asked for).  Returns after enqueueing; synchronise the stream before reading. */
+jefi_status jefi_fields_series_host(jefi_ctx* ctx, int32_t step_begin, int32_t step_count,
+                                    int64_t obs_begin, int64_t obs_count,
+                                    void* E_out_host, void* B_out_host, jefi_stream stream);
 
 /* Same for a time t that must lie on the step grid to within 1e-6*dt (the paper
  * evaluates at snapshots only), else JEFI_ERR_TIME_RANGE. */
@@ -150,9 +172,12 @@ jefi_status jefi_fields_at_time(jefi_ctx* ctx, double t, int64_t obs_begin, int6
 jefi_status jefi_fields_host(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t obs_count,
                              void* E_out_host, void* B_out_host, jefi_stream stream);
 
-/* Kernel selection for jefi_fields: 0 = automatic (tiled kernel for regular observation
- * grids, per-point kernel otherwise), 1 = always the per-point kernel (one thread per
- * observation point, the paper's shape PAPER.md:93), 2 = tiled kernel or JEFI_ERR_UNSUPPORTED. */
+/* Kernel selection: 0 = automatic (tiled kernels for regular observation grids -- one-step for
+ * jefi_fields, time-blocked for jefi_fields_series -- per-point kernel otherwise), 1 = always the
+ * per-point kernel (one thread per observation point, the paper's shape PAPER.md:93), 2 = the
+ * one-step tiled kernel or JEFI_ERR_UNSUPPORTED (jefi_fields_series then loops over it),
+ * 3 = like 0, but jefi_fields_series of at least half a block of steps must run the
+ * time-blocked kernel or fails with JEFI_ERR_UNSUPPORTED. */
 jefi_status jefi_set_kernel(jefi_ctx* ctx, int32_t which);
 
 /* Bytes of device memory owned by the context. */

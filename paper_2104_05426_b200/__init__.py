@@ -24,7 +24,7 @@ EXPORTS = (                                   # include/jefi.h: the product ABI
     "jefi_fields_at_time", "jefi_fields_host", "jefi_set_kernel",
     "jefi_device_bytes", "jefi_destroy", "jefi_status_string", "jefi_last_error",
     "jefi_flops_per_pair", "jefi_shard_obs",
-    "jefi_append_step", "jefi_append_step_host", "jefi_fields_series",
+    "jefi_append_step", "jefi_append_step_host", "jefi_fields_series", "jefi_fields_series_host",
 )
 INSTRUMENT_EXPORTS = (                        # include/jefi_instrument.h: bench / test instrumentation
     "jefi_launch_count", "jefi_measure_alu_peak", "jefi_debug_pair_lags", "jefi_debug_launch_limits",
@@ -67,6 +67,7 @@ _lib.jefi_append_step.argtypes = [_P, _P, _P, _P]
 _lib.jefi_append_step_host.argtypes = [_P, _P, _P, _P]
 _lib.jefi_fields.argtypes = [_P, C.c_int32, C.c_int64, C.c_int64, _P, _P, _P]
 _lib.jefi_fields_series.argtypes = [_P, C.c_int32, C.c_int32, C.c_int64, C.c_int64, _P, _P, _P]
+_lib.jefi_fields_series_host.argtypes = [_P, C.c_int32, C.c_int32, C.c_int64, C.c_int64, _P, _P, _P]
 _lib.jefi_fields_at_time.argtypes = [_P, C.c_double, C.c_int64, C.c_int64, _P, _P, _P]
 _lib.jefi_fields_host.argtypes = [_P, C.c_int32, C.c_int64, C.c_int64, _P, _P, _P]
 _lib.jefi_set_kernel.argtypes = [_P, C.c_int32]
@@ -171,6 +172,12 @@ def jefi_fields(ctx, step, obs_begin, obs_count, E_out_dev, B_out_dev, stream=No
 def jefi_fields_series(ctx, step_begin, step_count, obs_begin, obs_count, E_out_dev, B_out_dev, stream=None):
     _check(_lib.jefi_fields_series(ctx, int(step_begin), int(step_count), int(obs_begin), int(obs_count),
                                    _ptr(E_out_dev), _ptr(B_out_dev), _stream(stream)), ctx, "jefi_fields_series")
+
+
+def jefi_fields_series_host(ctx, step_begin, step_count, obs_begin, obs_count, E_out_host, B_out_host, stream=None):
+    _check(_lib.jefi_fields_series_host(ctx, int(step_begin), int(step_count), int(obs_begin), int(obs_count),
+                                        _ptr(E_out_host), _ptr(B_out_host), _stream(stream)), ctx,
+           "jefi_fields_series_host")
 
 
 def jefi_fields_at_time(ctx, t, obs_begin, obs_count, E_out_dev, B_out_dev, stream=None):
@@ -279,6 +286,11 @@ class Jefi:
     def fields_series(self, step_begin, step_count, E_out_dev, B_out_dev, obs_begin=0, obs_count=None, stream=None):
         n = self.n_points - obs_begin if obs_count is None else obs_count
         jefi_fields_series(self.ctx, step_begin, step_count, obs_begin, n, E_out_dev, B_out_dev, stream)
+
+    def fields_series_host(self, step_begin, step_count, E_out_host, B_out_host, obs_begin=0, obs_count=None,
+                           stream=None):
+        n = self.n_points - obs_begin if obs_count is None else obs_count
+        jefi_fields_series_host(self.ctx, step_begin, step_count, obs_begin, n, E_out_host, B_out_host, stream)
 
     def fields_host(self, step, E_out_host, B_out_host, obs_begin=0, obs_count=None, stream=None):
         n = self.n_points - obs_begin if obs_count is None else obs_count

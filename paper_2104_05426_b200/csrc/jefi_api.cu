@@ -45,7 +45,8 @@ jefi_status dev_alloc(jefi_ctx* c, void** p, size_t bytes, const char* what)
 void free_all(jefi_ctx* c)
 {
     cudaFree(c->hist); cudaFree(c->scratch); cudaFree(c->stage_E); cudaFree(c->stage_B);
-    cudaFree(c->series); cudaFree(c->raw_rho); cudaFree(c->raw_J); cudaFree(c->last); cudaFree(c->new_stage);
+    cudaFree(c->tiles.perm); cudaFree(c->tiles.boxes);
+    cudaFree(c->series); cudaFree(c->stage_series); cudaFree(c->raw_rho); cudaFree(c->raw_J); cudaFree(c->last); cudaFree(c->new_stage);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->ev_copied) cudaEventDestroy(c->ev_copied);
     if (c->ev_raw_free) cudaEventDestroy(c->ev_raw_free);
@@ -89,6 +90,7 @@ jefi_status run_fields(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t o
     int n = 0;
     if (ctx->kernel_choice != 1) {
         n = jefi::launch_fields_tiled(ctx->P, ctx->dtype, ctx->hist, L);
+        if (n == 0) n = jefi::launch_fields_list(ctx->P, ctx->dtype, ctx->hist, L, ctx->tiles);
         if (n == 0 && ctx->kernel_choice == 2) {
             set_err(ctx, "tiled kernel does not support this request", cudaSuccess);
             return JEFI_ERR_UNSUPPORTED;
@@ -170,6 +172,23 @@ jefi_status jefi_create(const jefi_grid_desc* src, const jefi_obs_desc* obs,
         (s = dev_alloc(c, &c->stage_E, (size_t)P.n_obs * 3 * c->elem, "cudaMalloc(E staging)")) != JEFI_OK ||
         (s = dev_alloc(c, &c->stage_B, (size_t)P.n_obs * 3 * c->elem, "cudaMalloc(B staging)")) != JEFI_OK) {
         free_all(c); delete c; return s;
+    }
+    if (obs->kind == 1 && P.n_obs > 0 && P.n_obs < (1LL << 31)) {
+        // explicit points: sort them into spatially compact tiles for the tiled kernel (pairwise_list.cu)
+        jefi::PointTiles& t = c->tiles;
+        t.tile_points = jefi::list_tile_points(dtype);
+        t.ntiles = (P.n_obs + t.tile_points - 1) / t.tile_points;
+        if ((s = dev_alloc(c, (void**)&t.perm, (size_t)P.n_obs * sizeof(int), "cudaMalloc(point permutation)")) != JEFI_OK ||
+            (s = dev_alloc(c, (void**)&t.boxes, (size_t)t.ntiles * 6 * sizeof(double), "cudaMalloc(tile boxes)")) != JEFI_OK) {
+            free_all(c); delete c; return s;
+        }
+        const int n = jefi::build_point_tiles(P, dtype, t);
+        if (n < 0) {
+            cudaGetLastError();
+            free_all(c); delete c;
+            return n == -2 ? JEFI_ERR_INVALID_ARG : JEFI_ERR_CUDA;
+        }
+        c->launches += n;
     }
     *out = c;
     return JEFI_OK;
@@ -389,6 +408,37 @@ jefi_status jefi_fields_host(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int
         return cuda_fail(ctx, "cudaMemcpyAsync(E)", e);
     if ((e = cudaMemcpyAsync(B_out_host, ctx->stage_B, bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
         return cuda_fail(ctx, "cudaMemcpyAsync(B)", e);
+    return JEFI_OK;
+}
+
+jefi_status jefi_fields_series_host(jefi_ctx* ctx, int32_t step_begin, int32_t step_count, int64_t obs_begin,
+                                    int64_t obs_count, void* E_out_host, void* B_out_host, jefi_stream stream)
+{
+    if (!ctx) return JEFI_ERR_INVALID_ARG;
+    if (step_count < 0) { set_err(ctx, "negative step count", cudaSuccess); return JEFI_ERR_INVALID_ARG; }
+    if (step_count == 0) return JEFI_OK;
+    jefi_status s = check_fields_args(ctx, step_begin, obs_begin, obs_count, E_out_host, B_out_host);
+    if (s != JEFI_OK) return s;
+    if (obs_count == 0) return JEFI_OK;
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e != cudaSuccess) return cuda_fail(ctx, "cudaSetDevice", e);
+    const size_t half = (size_t)step_count * 3 * (size_t)obs_count * ctx->elem;
+    if (ctx->stage_series_bytes < 2 * half) {
+        // (growing frees the old staging: wait for the copies still reading it)
+        if (ctx->stage_series) { cudaDeviceSynchronize(); cudaFree(ctx->stage_series); ctx->dev_bytes -= (long long)ctx->stage_series_bytes; }
+        ctx->stage_series = nullptr; ctx->stage_series_bytes = 0;
+        if ((s = dev_alloc(ctx, &ctx->stage_series, 2 * half, "cudaMalloc(series staging)")) != JEFI_OK) return s;
+        ctx->stage_series_bytes = 2 * half;
+    }
+    char* Ed = (char*)ctx->stage_series;
+    char* Bd = Ed + half;
+    s = jefi_fields_series(ctx, step_begin, step_count, obs_begin, obs_count, Ed, Bd, stream);
+    if (s != JEFI_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((e = cudaMemcpyAsync(E_out_host, Ed, half, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+        return cuda_fail(ctx, "cudaMemcpyAsync(E series)", e);
+    if ((e = cudaMemcpyAsync(B_out_host, Bd, half, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+        return cuda_fail(ctx, "cudaMemcpyAsync(B series)", e);
     return JEFI_OK;
 }
 

@@ -44,6 +44,24 @@ struct FieldsLaunch {
     cudaStream_t stream;
 };
 
+// Explicit point lists on the tiled path (pairwise_list.cu): jefi_create sorts the points into
+// spatially compact tiles -- perm[s] = original index of entry s of the sorted order,
+// boxes[tile][6] = min xyz, max xyz of the tile relative to source cell (0,0,0)
+struct PointTiles {
+    int*      perm;
+    double*   boxes;
+    long long ntiles;
+    int       tile_points;
+    double    max_diam;     // longest tile-box diagonal
+    double    far;          // bound on the distance between any point and any source cell
+};
+int list_tile_points(jefi_dtype dt);
+// synchronous; returns kernels launched, -1 on a CUDA error, -2 on non-finite positions
+int build_point_tiles(const Params& P, jefi_dtype dt, PointTiles& pt);
+// whole-list requests only; returns 0 if it does not support the request
+struct FieldsLaunch;
+int launch_fields_list(const Params& P, jefi_dtype dt, const void* hist, const FieldsLaunch& L, const PointTiles& pt);
+
 // each returns the number of kernels it launched (>0) or a negative value on a launch error,
 // leaving the CUDA error in cudaGetLastError()/cudaPeekAtLastError()
 int launch_prepass(const Params& P, jefi_dtype dt, const void* rho, const void* J, void* hist,
@@ -83,6 +101,9 @@ struct jefi_ctx {
     long long    chunk_bytes;      // packed-history bytes per source chunk (L2 sharing, pairwise_tiled.cu)
     void*        stage_E;          // device staging for jefi_fields_host, [3][N_o]
     void*        stage_B;
+    void*        stage_series;     // device staging for jefi_fields_series_host (lazy, grows), E then B
+    size_t       stage_series_bytes;
+    jefi::PointTiles tiles;        // kind 1 observation sets: the tiling built by jefi_create
     void*        series;           // series layout of the history (lazy: first jefi_fields_series), [N_s][units][T+3]
     bool         series_valid;     // matches the packed history
     void*        last;             // raw values of the two newest stored steps, [2][4][N_s]

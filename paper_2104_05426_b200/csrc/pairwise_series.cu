@@ -131,27 +131,45 @@ __device__ __forceinline__ void load_raw(unsigned addr, unsigned unit_off, doubl
     v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
 }
 
-// one pair, NS steps.  NL = slots loaded: NS + 2 (centred), NS + 1 (backward)
-template <typename T, int NS, bool SLOW, bool EDGE, bool BACKWARD>
-__device__ __forceinline__ void pair_series(SAcc<T, NS>& a, T ox, T ryz, unsigned C, T sx, T neg_inv_cdt, T rcut2,
-                                            T inv_kappa, int n0, unsigned unit_off)
+// per-launch constants in the kernel's own precision (kernel parameters live in the constant
+// bank: the FMA-pipe instructions take them as operands without a register read)
+template <typename T> struct SConsts { T neg_inv_cdt, rcut2, inv_kappa, shy, shz; };
+
+// geometry of one pair: the slot address of its first record, the screening weight, dx
+template <typename T> struct SGeo { unsigned addr; T w, dx; int m0; };
+
+template <typename T, bool SLOW, bool EDGE>
+__device__ __forceinline__ SGeo<T> series_geo(T ox, T ryz, unsigned meta_addr, const SConsts<T>& k, int n0)
 {
-    T dx, w;
+    unsigned C;
+    T sx;
+    if constexpr (sizeof(T) == 4) {
+        const float4 mv = lds128(meta_addr);
+        C = __float_as_uint(mv.x); sx = mv.y;
+    } else {
+        const double2 mv = lds128d(meta_addr);
+        C = (unsigned)__double2loint(mv.x); sx = mv.y;
+    }
+    SGeo<T> G;
     unsigned bits;
-    pair_geo<T, SLOW>(ox, sx, ryz, neg_inv_cdt, rcut2, dx, w, bits);
-    const unsigned addr = C + (bits << 4);
-    constexpr int NL = BACKWARD ? NS + 1 : NS + 2;
-    T r[NL][4];
-#pragma unroll
-    for (int i = 0; i < NL; ++i) load_raw(addr + 16u * i, unit_off, r[i]);
+    pair_geo<T, SLOW>(ox, sx, ryz, k.neg_inv_cdt, k.rcut2, G.dx, G.w, bits);
+    G.addr = C + (bits << 4);
+    G.m0 = EDGE ? n0 - lag_of_bits(bits, Prec<T>::kMagicLo) : 0;
+    return G;
+}
+
+// one pair, NS steps.  NL = slots loaded: NS + 2 (centred), NS + 1 (backward)
+template <typename T, int NS, bool EDGE, bool BACKWARD>
+__device__ __forceinline__ void series_accumulate(SAcc<T, NS>& a, const SGeo<T>& G, T inv_kappa, unsigned unit_off,
+                                                  const T (&r)[BACKWARD ? NS + 1 : NS + 2][4])
+{
+    const T w = G.w;
     const T g = w * w;
-    const T h = dx * g;
+    const T h = G.dx * g;
     const T wq = w * inv_kappa;
-    int m0 = 0;
-    if (EDGE) m0 = n0 - lag_of_bits(bits, Prec<T>::kMagicLo);
 #pragma unroll
     for (int i = 0; i < NS; ++i) {
-        if (EDGE && m0 + i < 0) continue;            // before the stored history: zero contribution (Q4)
+        if (EDGE && G.m0 + i < 0) continue;          // before the stored history: zero contribution (Q4)
         const T* v = r[i + 1];
         T d[4];
 #pragma unroll
@@ -173,22 +191,24 @@ __device__ __forceinline__ void pair_series(SAcc<T, NS>& a, T ox, T ryz, unsigne
     }
 }
 
+// One source row (or the part of it in this stage).  Software pipeline: the geometry of cell
+// c+1 (meta load -> distance -> MUFU -> lag -> address: one long dependency chain) is computed
+// beside the record loads and the accumulation of cell c.  The look-ahead past the last cell
+// reads a meta slot that may be stale; its geometry is computed and never used.
 template <typename T, int NS, bool SLOW, bool EDGE, bool BACKWARD>
-__device__ __forceinline__ void row_series(SAcc<T, NS>& a, T ox, T ryz, unsigned meta_addr, int len, T neg_inv_cdt,
-                                           T rcut2, T inv_kappa, int n0, unsigned unit_off)
+__device__ __forceinline__ void row_series(SAcc<T, NS>& a, T ox, T ryz, unsigned meta_addr, int len,
+                                           const SConsts<T>& k, int n0, unsigned unit_off)
 {
+    constexpr int NL = BACKWARD ? NS + 1 : NS + 2;
+    SGeo<T> G = series_geo<T, SLOW, EDGE>(ox, ryz, meta_addr, k, n0);
 #pragma unroll 1
     for (int c = 0; c < len; ++c) {
-        unsigned C;
-        T sx;
-        if constexpr (sizeof(T) == 4) {
-            const float4 mv = lds128(meta_addr + c * 16u);
-            C = __float_as_uint(mv.x); sx = mv.y;
-        } else {
-            const double2 mv = lds128d(meta_addr + c * 16u);
-            C = (unsigned)__double2loint(mv.x); sx = mv.y;
-        }
-        pair_series<T, NS, SLOW, EDGE, BACKWARD>(a, ox, ryz, C, sx, neg_inv_cdt, rcut2, inv_kappa, n0, unit_off);
+        T r[NL][4];
+#pragma unroll
+        for (int i = 0; i < NL; ++i) load_raw(G.addr + 16u * i, unit_off, r[i]);
+        const SGeo<T> Gn = series_geo<T, SLOW, EDGE>(ox, ryz, meta_addr + (c + 1) * 16u, k, n0);
+        series_accumulate<T, NS, EDGE, BACKWARD>(a, G, k.inv_kappa, unit_off, r);
+        G = Gn;
     }
 }
 
@@ -210,7 +230,8 @@ __device__ __forceinline__ void fold_row_series(SAcc<T, NS>& a, T dy, T dz)
 // producer warp; grid.x = tile + ntiles * (step block), grid.y = source chunk.
 template <typename T, int NS, int TX, int TY, int TZ, int CW, int CTAS, bool BACKWARD>
 __global__ void __launch_bounds__((CW + 1) * 32, CTAS)
-fields_series_kernel(const uint4* __restrict__ hist, double* __restrict__ partial, const SeriesArgs a)
+fields_series_kernel(const uint4* __restrict__ hist, double* __restrict__ partial, const SeriesArgs a,
+                     const SConsts<T> k)
 {
     constexpr int U = SPrec<T>::U;
     static_assert(TX == 8 && TY % 4 == 0 && TX * TY * TZ == CW * 32, "a warp covers 8 x 4 points of one z layer");
@@ -246,7 +267,7 @@ fields_series_kernel(const uint4* __restrict__ hist, double* __restrict__ partia
         const double bz0 = a.d0z + iz0 * a.ohz, bz1 = bz0 + a.box_hz;
         for (int it = 0; it < nst; ++it) {
             const int s = it % a.stages;
-            if (it >= a.stages) mbar_wait(sbase + kOffEmpty + 8 * s, ((it / a.stages) - 1) & 1);
+            if (it >= a.stages) mbar_wait_parked(sbase + kOffEmpty + 8 * s, ((it / a.stages) - 1) & 1);
             const long long j = cb + (long long)it * a.cps + lane;
             const bool valid = lane < a.cps && j < ce;
             int flags = 0, p_src = 0, cnt = 0, nz = 0;
@@ -330,8 +351,6 @@ fields_series_kernel(const uint4* __restrict__ hist, double* __restrict__ partia
     // tile's windows) and store nothing
     ix = ix < a.nox ? ix : a.nox - 1; iy = iy < a.noy ? iy : a.noy - 1; iz = iz < a.noz ? iz : a.noz - 1;
     const T ox = obs_coord<T>(a.d0x, ix, a.ohx), oy = obs_coord<T>(a.d0y, iy, a.ohy), oz = obs_coord<T>(a.d0z, iz, a.ohz);
-    const T shy = (T)a.shy, shz = (T)a.shz, rcut2 = (T)a.rcut2, inv_kappa = (T)a.inv_kappa;
-    const T neg_inv_cdt = tie_biased_neg_inv_cdt<T>(a.inv_cdt);
     SAcc<T, NS> acc;
 #pragma unroll
     for (int i = 0; i < NS; ++i) {
@@ -355,13 +374,13 @@ fields_series_kernel(const uint4* __restrict__ hist, double* __restrict__ partia
             int len = a.nsx - jx;
             len = len < cnt - pos ? len : cnt - pos;
             T dy, dz;
-            const T ryz = row_ryz<T>(oy, oz, jy, jz, shy, shz, dy, dz);
+            const T ryz = row_ryz<T>(oy, oz, jy, jz, k.shy, k.shz, dy, dz);
             const unsigned meta_addr = sbase + kOffMeta + (unsigned)(s * kStageCells + pos) * 16u;
             switch (flags) {
-                case 0:  row_series<T, NS, false, false, BACKWARD>(acc, ox, ryz, meta_addr, len, neg_inv_cdt, rcut2, inv_kappa, n0, unit_off); break;
-                case 1:  row_series<T, NS, true,  false, BACKWARD>(acc, ox, ryz, meta_addr, len, neg_inv_cdt, rcut2, inv_kappa, n0, unit_off); break;
-                case 2:  row_series<T, NS, false, true,  BACKWARD>(acc, ox, ryz, meta_addr, len, neg_inv_cdt, rcut2, inv_kappa, n0, unit_off); break;
-                default: row_series<T, NS, true,  true,  BACKWARD>(acc, ox, ryz, meta_addr, len, neg_inv_cdt, rcut2, inv_kappa, n0, unit_off); break;
+                case 0:  row_series<T, NS, false, false, BACKWARD>(acc, ox, ryz, meta_addr, len, k, n0, unit_off); break;
+                case 1:  row_series<T, NS, true,  false, BACKWARD>(acc, ox, ryz, meta_addr, len, k, n0, unit_off); break;
+                case 2:  row_series<T, NS, false, true,  BACKWARD>(acc, ox, ryz, meta_addr, len, k, n0, unit_off); break;
+                default: row_series<T, NS, true,  true,  BACKWARD>(acc, ox, ryz, meta_addr, len, k, n0, unit_off); break;
             }
             pos += len; jx += len;
             const bool row_done = jx == a.nsx;
@@ -440,6 +459,9 @@ int launch_series_shape(const Params& P, jefi_dtype dt, const void* series, cons
     a.inv_cdt = 1.0 / (P.c * P.dt);
     const double kappa = (BACKWARD ? 1.0 : 0.5) * a.inv_cdt;
     a.inv_kappa = 1.0 / kappa;
+    SConsts<T> k;
+    k.neg_inv_cdt = tie_biased_neg_inv_cdt<T>(a.inv_cdt); k.rcut2 = (T)a.rcut2; k.inv_kappa = (T)a.inv_kappa;
+    k.shy = (T)P.sh[1]; k.shz = (T)P.sh[2];
     a.Tq = P.T + 3;
     a.tiles_x = (P.no[0] + TX - 1) / TX;
     a.tiles_y = (P.no[1] + TY - 1) / TY;
@@ -534,7 +556,7 @@ int launch_series_shape(const Params& P, jefi_dtype dt, const void* series, cons
             a.chunk_base = (int)base;
             a.accumulate = base > 0 ? 1 : 0;
             dim3 grid((unsigned)nct, (unsigned)sl);
-            kern<<<grid, kThreads, smem, L.stream>>>((const uint4*)series, (double*)L.scratch, a);
+            kern<<<grid, kThreads, smem, L.stream>>>((const uint4*)series, (double*)L.scratch, a, k);
             if (cudaPeekAtLastError() != cudaSuccess) return -1;
             ++launches;
         }
@@ -580,13 +602,18 @@ int launch_series_layout(const Params& P, jefi_dtype dt, const void* packed, voi
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
-int series_block_steps(jefi_dtype dt) { return dt == JEFI_F32 ? 8 : 4; }
+int series_block_steps(jefi_dtype dt) { return dt == JEFI_F32 ? 6 : 4; }
 
 int launch_fields_series(const Params& P, jefi_dtype dt, const void* series, const FieldsLaunch& L, int step_begin,
                          int step_count)
 {
     if (P.obs_kind != 0) return 0;
-    if (dt == JEFI_F32) return launch_series_T<float, 8, 3>(P, dt, series, L, step_begin, step_count);
+    // Block length NS and CTAs per SM, measured on c4 (128 steps, ms per series) and the paper's X1
+    // series (411 steps on 15^3).  fp32, (NS, CTAs/SM, geometry look-ahead): (8,3,no) 894 / 10.5,
+    // (8,3,yes: spills) 1026 / 10.2, (8,2,no) 929 / 9.9, (8,2,yes) 851 / 9.0, (6,3,no) 957 / 8.8,
+    // (6,3,yes) 871 / 7.9, (4,3,no) 996; a 256-point tile, one CTA per SM: 933.  fp64 on c4:
+    // (4,2,no) 1875, (4,2,yes) 1784, (2,3,yes) 1961, (6,1,yes) 1902, (4,1,yes) 2066, (3,2,yes) 1830.
+    if (dt == JEFI_F32) return launch_series_T<float, 6, 3>(P, dt, series, L, step_begin, step_count);
     return launch_series_T<double, 4, 2>(P, dt, series, L, step_begin, step_count);
 }
 

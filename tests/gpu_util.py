@@ -10,6 +10,8 @@ def torch_dtype(w):
 
 def make_ctx(w, jb, deriv_mode=0, points=None):
     import torch
+    if points is None and getattr(w, "points", None) is not None:
+        points = w.points
     if points is None:
         return jb.Jefi(w.n_src, w.origin_src, w.spacing_src, dt=w.dt, c=w.c, nsteps=w.T, dtype=w.dtype,
                        n_obs=w.n_obs, origin_obs=w.origin_obs, spacing_obs=w.spacing_obs, t0=w.t0,

@@ -7,7 +7,7 @@ import pytest
 
 import workloads as wl
 from conftest import rel_l2
-from gpu_util import gpu_fields, make_ctx, oracle_fields, tol_for, upload
+from gpu_util import gpu_fields, gpu_fields_series, make_ctx, oracle_fields, tol_for, upload
 
 pytestmark = pytest.mark.gpu
 
@@ -209,20 +209,102 @@ def test_obs_subranges_match_the_full_call(jb, kernel):
         ctx.close()
 
 
+@pytest.mark.parametrize("kernel", [1, 2])
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-def test_explicit_point_list_matches_oracle(jb, dtype):
+def test_explicit_point_list_matches_oracle(jb, dtype, kernel):
+    """257 unstructured points (one ragged tile), per-point kernel and tiled list kernel (kernel 2 =
+    tiled or JEFI_ERR_UNSUPPORTED).  fp64: white-noise history.  fp32: the same noise modulated
+    smoothly in time -- on unstructured geometry a pair can sit within the fp32 error of a lag tie,
+    where either step is as good a nearest snapshot but white noise would turn the choice into an
+    O(1) error of that term (workloads.modulate_in_time)."""
     w = wl.random_history((7, 6, 5), 32, seed=13, dtype=dtype, dt=0.03)
+    if dtype == "f32":
+        w = wl.modulate_in_time(w, 32.0)
     u = wl.uniform01(4242, 0, 3 * 257).reshape(257, 3)
     pts = (u - 0.5) * np.array([1.5, 1.2, 2.0])
     pts = pts.astype(w.np_dtype).astype(np.float64)     # both sides see the same rounded points
     ctx = make_ctx(w, jb, points=pts)
     try:
+        ctx.set_kernel(kernel)
         upload(ctx, w)
-        E, B = gpu_fields(ctx, w, 31)
-        Eo, Bo = oracle_fields(w, 31, points=pts)
-        check(w, E, B, Eo, Bo, None, "point list")
+        for step in (31, 9):
+            E, B = gpu_fields(ctx, w, step)
+            Eo, Bo = oracle_fields(w, step, points=pts)
+            check(w, E, B, Eo, Bo, None, f"point list kernel {kernel} step {step}")
     finally:
         ctx.close()
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_point_list_tiled_every_point_against_the_oracle(jb, dtype):
+    """20 000 unstructured points (40 / 79 tiles, the last ragged) in and around the 32^3 source grid
+    of configs[1]: EVERY output of the tiled list kernel against the oracle; the outputs come
+    back in the caller's order although the kernel works through a Morton-sorted permutation;
+    sub-ranges (served by the per-point kernel) agree with the full call."""
+    w = wl.config2c_noise(dtype)
+    if dtype == "f32":
+        w = wl.modulate_in_time(w, 64.0)
+    w = wl.with_random_points(w, 20000, margin=0.3)
+    ctx = make_ctx(w, jb)
+    try:
+        ctx.set_kernel(2)
+        upload(ctx, w)
+        E, B = gpu_fields(ctx, w, 63)
+        Eo, Bo = oracle_fields(w, 63, points=w.points)
+        check(w, E, B, Eo, Bo, None, f"point list 20000 {dtype}")
+        ctx.set_kernel(0)
+        e, b = gpu_fields(ctx, w, 63, 1234, 4321)
+        tol = tol_for(w)
+        assert max(rel_l2(e, E[:, 1234:5555], field_ref=E[:, 1234:5555])) <= 2 * tol
+        assert max(rel_l2(b, B[:, 1234:5555], field_ref=B[:, 1234:5555])) <= 2 * tol
+    finally:
+        ctx.close()
+
+
+def test_point_list_at_c3_scale_and_degenerate_sets(jb):
+    """65 536 unstructured points on the 64^3 x 221-step collision history (fp32, the bench workload
+    c3_points): the oracle on 8192 seeded points, every other output against the per-point kernel.
+    Then the degenerate sets: all points identical (one bin, zero-size boxes), points on a line,
+    a single point."""
+    w = wl.with_random_points(wl.config3_collision(), 65536)
+    ctx = make_ctx(w, jb)
+    try:
+        upload(ctx, w)
+        ctx.set_kernel(2)
+        E, B = gpu_fields(ctx, w, 220)
+        idx = w.obs_subset(8192)
+        Eo, Bo = oracle_fields(w, 220, points=w.points[idx])
+        check(w, E[:, idx], B[:, idx], Eo, Bo, None, "c3 points")
+        ctx.set_kernel(1)
+        E1, B1 = gpu_fields(ctx, w, 220)
+        for got, ref, name in ((E, E1, "E"), (B, B1, "B")):
+            rms = np.sqrt(np.mean(np.sum(ref * ref, axis=0)))
+            assert np.abs(got - ref).max() <= 4e-3 * rms, name
+            assert max(rel_l2(got, ref, field_ref=ref)) <= 4e-4
+    finally:
+        ctx.close()
+    w = wl.random_history((6, 5, 4), 24, seed=15, dtype="f64", dt=0.05)
+    for pts in (np.tile([[0.31, -0.2, 0.45]], (700, 1)),
+                np.stack([np.linspace(-2, 2, 1500), np.full(1500, 0.4), np.full(1500, -0.3)], axis=1),
+                np.array([[0.0, 0.0, 1.0]])):
+        ctx = make_ctx(w, jb, points=pts)
+        try:
+            ctx.set_kernel(2)
+            upload(ctx, w)
+            E, B = gpu_fields(ctx, w, 23)
+            Eo, Bo = oracle_fields(w, 23, points=pts)
+            check(w, E, B, Eo, Bo, None, f"degenerate list of {len(pts)}")
+        finally:
+            ctx.close()
+
+
+def test_point_list_rejects_non_finite_positions(jb):
+    import torch
+    w = wl.random_history((4, 4, 4), 8, seed=1, dtype="f32")
+    pts = np.zeros((10, 3)); pts[3, 1] = np.nan
+    with pytest.raises(jb.JefiError) as e:
+        make_ctx(w, jb, points=pts)
+    assert e.value.status == jb.JEFI_ERR_INVALID_ARG
 
 
 def test_time_series_and_truncated_history(jb):
@@ -784,5 +866,46 @@ def test_source_chunks_spread_over_accumulating_launches(jb, dtype):
         check(w, E0, B0, Eo, Bo, None, f"single launch {dtype}")
         E1, B1 = gpu_fields(ctx, w, 59, 100, 333)               # a sub-range through the same path
         np.testing.assert_allclose(E1, E[:, 100:433], rtol=1e-4, atol=1e-5 * np.abs(E).max())
+    finally:
+        ctx.close()
+
+
+# ------------------------------------------------------------------ N ranks, ONE problem (bench.py --scaling strong)
+@pytest.mark.parametrize("world", [2, 3, 8])
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_strong_scaling_slices_concatenate_to_the_full_evaluation(jb, world, dtype):
+    """SURVEY.md 8(e) / 8(f)-4, the paper's S-O decomposition with one source region (PAPER.md:95-101,
+    Fig. 2): the observation set is partitioned over `world` ranks (jefi_shard_obs), the history is
+    replicated, every rank evaluates its slice; there is nothing to reduce.  Only one GPU is
+    available, so the ranks' calls run one after another on it: the concatenation in rank order must
+    equal the unsharded call (to tolerance -- the launcher picks a different source-chunk count per
+    slice, so the summation order differs) and the oracle; the same for a time series."""
+    w = wl.random_history((10, 9, 8), 40, seed=91, dtype=dtype, n_obs=(16, 12, 10), dt=0.05)
+    obs = jb.make_obs_grid(w.n_obs, w.origin_obs, w.spacing_obs)
+    ctx = make_ctx(w, jb)
+    try:
+        upload(ctx, w)
+        E, B = gpu_fields(ctx, w, 39)
+        Es, Bs = gpu_fields_series(ctx, w, 30, 10)
+        parts, sparts, pos = [], [], 0
+        for r in range(world):
+            b, c = jb.jefi_shard_obs(obs, r, world)
+            assert b == pos
+            pos += c
+            parts.append(gpu_fields(ctx, w, 39, b, c))
+            sparts.append(gpu_fields_series(ctx, w, 30, 10, b, c))
+        assert pos == w.N_o
+        Ec = np.concatenate([p[0] for p in parts], axis=1)
+        Bc = np.concatenate([p[1] for p in parts], axis=1)
+        tol = tol_for(w)
+        assert max(rel_l2(Ec, E, field_ref=E)) <= tol and max(rel_l2(Bc, B, field_ref=B)) <= tol
+        Eo, Bo = oracle_fields(w, 39)
+        check(w, Ec, Bc, Eo, Bo, None, f"strong x{world} {dtype}")
+        Esc = np.concatenate([p[0] for p in sparts], axis=2)
+        Bsc = np.concatenate([p[1] for p in sparts], axis=2)
+        for k in (0, 9):
+            assert max(rel_l2(Esc[k], Es[k], field_ref=Es[k])) <= tol
+            Eo, Bo = oracle_fields(w, 30 + k)
+            check(w, Esc[k], Bsc[k], Eo, Bo, None, f"strong x{world} {dtype} series step {30 + k}")
     finally:
         ctx.close()

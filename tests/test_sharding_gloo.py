@@ -1,7 +1,9 @@
 """N > 1 host logic on CPU: world_size 2 over the gloo backend (no GPU).
 
 The method has no exchange step: ranks either run one S-O pair each
-(bench.py --gpus N) or partition one observation set with jefi_shard_obs.  Covered here:
+(bench.py --gpus N) or share ONE problem (--scaling strong): rank 0's raw history is broadcast,
+the observation set is partitioned with jefi_shard_obs, the results are disjoint slices.  Covered here:
+the broadcast + slice logic of the strong mode (the functions bench.py itself calls),
 the partition rule (disjoint, ordered, complete, whole z-layers), that evaluating the slices
 separately and concatenating them in rank order equals the unsharded evaluation (the oracle
 stands in for the kernels: this test is about the slicing, not the arithmetic), and the
@@ -33,10 +35,18 @@ def _worker(rank, world, port, out_dir):
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
         w = wl.random_history((5, 4, 3), 12, seed=3, dtype="f64", n_obs=(4, 3, 5), dt=0.05)
+        # bench.py --scaling strong, host side: only rank 0 holds the raw history; the others
+        # receive it through bench.broadcast_history, then every rank evaluates ITS slice of the
+        # one observation set (bench.strong_slice -> jefi_shard_obs)
+        rho = torch.from_numpy(w.rho.copy()) if rank == 0 else torch.zeros(w.rho.shape, dtype=torch.float64)
+        J = torch.from_numpy(w.J.copy()) if rank == 0 else torch.zeros(w.J.shape, dtype=torch.float64)
+        bench.broadcast_history(rho, J)
+        assert np.array_equal(rho.numpy(), w.rho) and np.array_equal(J.numpy(), w.J)
+        begin, count = bench.strong_slice(jb, w, rank, world)
         obs = jb.make_obs_grid(w.n_obs, w.origin_obs, w.spacing_obs)
-        begin, count = jb.jefi_shard_obs(obs, rank, world)
+        assert (begin, count) == jb.jefi_shard_obs(obs, rank, world)
         idx = np.arange(begin, begin + count)
-        E, B = oracle.fields(w.n_src, w.origin_src, w.spacing_src, w.rho, w.J, dt=w.dt, c=w.c, step=11,
+        E, B = oracle.fields(w.n_src, w.origin_src, w.spacing_src, rho.numpy(), J.numpy(), dt=w.dt, c=w.c, step=11,
                              obs_xyz=w.obs_points(idx), nthreads=1)
         # gather the slices (sizes differ by a z-layer: pad to the largest)
         sizes = [torch.zeros(1, dtype=torch.int64) for _ in range(world)]

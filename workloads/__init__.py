@@ -58,6 +58,7 @@ class Workload:
     c: float = 1.0
     t0: float = 0.0
     seed: int = BASE_SEED
+    points: np.ndarray = field(repr=False, default=None)   # explicit observation points [n,3] instead of a grid
 
     @property
     def origin_src(self):
@@ -69,7 +70,7 @@ class Workload:
 
     @property
     def N_o(self) -> int:
-        return int(np.prod(self.n_obs))
+        return int(self.points.shape[0]) if self.points is not None else int(np.prod(self.n_obs))
 
     @property
     def pairs_per_step(self) -> int:
@@ -79,6 +80,8 @@ class Workload:
         """float64 [n,3] positions of linear obs indices (x fastest); all points if idx is None."""
         nx, ny, nz = self.n_obs
         idx = np.arange(self.N_o, dtype=np.int64) if idx is None else np.asarray(idx, dtype=np.int64)
+        if self.points is not None:
+            return np.ascontiguousarray(self.points[idx], dtype=np.float64)
         ix, iy, iz = idx % nx, (idx // nx) % ny, idx // (nx * ny)
         p = np.empty((idx.size, 3), dtype=np.float64)
         for a, i in enumerate((ix, iy, iz)):
@@ -87,6 +90,11 @@ class Workload:
 
     def obs_subset(self, count: int, seed_offset: int = 0) -> np.ndarray:
         """Seeded subset of linear obs indices: 8 corners, centre, 6 face centres, rest random."""
+        if self.points is not None:
+            if count >= self.N_o:
+                return np.arange(self.N_o, dtype=np.int64)
+            u = uniform01(self.seed + 7919 + seed_offset, 0, count)
+            return np.unique(np.minimum((u * self.N_o).astype(np.int64), self.N_o - 1))
         nx, ny, nz = self.n_obs
         lin = lambda i, j, k: (k * ny + j) * nx + i
         fixed = [lin(i, j, k) for i in (0, nx - 1) for j in (0, ny - 1) for k in (0, nz - 1)]
@@ -283,3 +291,57 @@ def random_history(n_src, T: int, seed: int, dtype: str = "f64", spacing=(0.1, 0
     rho = (2 * uniform01(seed, 0, T * Ns) - 1).reshape(T, nz, ny, nx)
     J = (2 * uniform01(seed + 1, 0, T * 3 * Ns) - 1).reshape(T, 3, nz, ny, nx)
     return _finish(w, rho, J)
+
+
+def paper_table4_largest(n: int = 160, T: int = 500, dtype: str = "f32") -> Workload:
+    """The paper's largest timed configuration, ntg = [160^3, 160^3], lts = 500 (PAPER.md:254,
+    Table 4 lower; dx = 0.1, c dt = 0.05 as in configs[4], so the longest lag exceeds the history).
+    The raw history is 33 GB in fp32: only one seeded snapshot (uniform [-1,1]) is generated on the
+    host; ``device_history(torch)`` fills the device arrays with that snapshot shifted by m cells
+    along x at step m (a copy per step, no arithmetic).  ``lazy`` tells bench.py that there are
+    no host arrays (no end-to-end leg, no oracle sample)."""
+    dx, dt = 0.1, 0.05
+    w = Workload(f"paper_table4_{n}", (n,) * 3, (dx,) * 3, (n,) * 3, (dx,) * 3, (-(n - 1) / 2 * dx,) * 3,
+                 dt, T, (T - 1,), dtype, seed=BASE_SEED + 160)
+    w.lazy = True
+
+    def device_history(torch):
+        base = (2 * uniform01(w.seed, 0, 4 * n ** 3) - 1).reshape(4, n, n, n).astype(w.np_dtype)
+        b = torch.from_numpy(base).cuda()
+        rho = torch.empty((T, n, n, n), dtype=b.dtype, device="cuda")
+        J = torch.empty((T, 3, n, n, n), dtype=b.dtype, device="cuda")
+        for m in range(T):
+            rho[m] = torch.roll(b[0], m, dims=2)
+            J[m] = torch.roll(b[1:], m, dims=3)
+        return rho, J
+
+    w.device_history = device_history
+    return w
+
+
+def with_random_points(w: Workload, n: int, seed_offset: int = 0, margin: float = 0.0) -> Workload:
+    """Replaces the observation grid of ``w`` by ``n`` seeded points, uniform in the box of the
+    source grid (grown by ``margin`` on every side), rounded to the run dtype so that both sides
+    see the same positions.  Unstructured observation sets are what detector positions or
+    particle positions of a coupled solver look like."""
+    half = [(a - 1) / 2.0 * h + 0.5 * h + margin for a, h in zip(w.n_src, w.spacing_src)]
+    u = uniform01(w.seed + 4242 + seed_offset, 0, 3 * n).reshape(n, 3)
+    pts = (2.0 * u - 1.0) * np.array(half)
+    w.points = pts.astype(w.np_dtype).astype(np.float64)
+    w.name = f"{w.name}_points{n}"
+    w.n_obs = (n, 1, 1)
+    return w
+
+
+def modulate_in_time(w: Workload, period: float, depth: float = 0.3) -> Workload:
+    """Multiplies every cell's history by 1 + depth*sin(2 pi m / period): white in space, smooth in
+    time.  For fp32 parity on UNSTRUCTURED geometry: there a pair can sit within the fp32 rounding
+    error of a retarded-index tie, and with a history that is white in time one flipped index is
+    an O(1) error in its term although either neighbouring step is an equally good nearest
+    snapshot ('harmless for smooth histories')."""
+    m = np.arange(w.T, dtype=np.float64)
+    f = 1.0 + depth * np.sin(2.0 * np.pi * m / period)
+    w.rho = np.ascontiguousarray((w.rho.astype(np.float64) * f[:, None, None, None]).astype(w.np_dtype))
+    w.J = np.ascontiguousarray((w.J.astype(np.float64) * f[:, None, None, None, None]).astype(w.np_dtype))
+    w.name = f"{w.name}_mod{period:g}"
+    return w
