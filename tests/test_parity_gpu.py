@@ -213,13 +213,16 @@ def test_obs_subranges_match_the_full_call(jb, kernel):
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_explicit_point_list_matches_oracle(jb, dtype, kernel):
     """257 unstructured points (one ragged tile), per-point kernel and tiled list kernel (kernel 2 =
-    tiled or JEFI_ERR_UNSUPPORTED).  fp64: white-noise history.  fp32: the same noise modulated
-    smoothly in time -- on unstructured geometry a pair can sit within the fp32 error of a lag tie,
-    where either step is as good a nearest snapshot but white noise would turn the choice into an
-    O(1) error of that term (workloads.modulate_in_time)."""
-    w = wl.random_history((7, 6, 5), 32, seed=13, dtype=dtype, dt=0.03)
+    tiled or JEFI_ERR_UNSUPPORTED).  fp64: white-noise history shorter than the longest lag.  fp32:
+    noise in space, smooth in time, history longer than the longest lag -- on unstructured geometry a
+    pair can sit within the fp32 error of a lag tie (here: point 184 / cell 185 has q = 31.499995),
+    where either step is as good a nearest snapshot, but white noise, or a history that starts
+    between the two candidates, turns the choice into an O(1) error of that term
+    (workloads.smooth_in_time; Q3)."""
     if dtype == "f32":
-        w = wl.modulate_in_time(w, 32.0)
+        w = wl.smooth_in_time(wl.random_history((7, 6, 5), 48, seed=13, dtype=dtype, dt=0.06), 48.0)
+    else:
+        w = wl.random_history((7, 6, 5), 32, seed=13, dtype=dtype, dt=0.03)
     u = wl.uniform01(4242, 0, 3 * 257).reshape(257, 3)
     pts = (u - 0.5) * np.array([1.5, 1.2, 2.0])
     pts = pts.astype(w.np_dtype).astype(np.float64)     # both sides see the same rounded points
@@ -227,7 +230,7 @@ def test_explicit_point_list_matches_oracle(jb, dtype, kernel):
     try:
         ctx.set_kernel(kernel)
         upload(ctx, w)
-        for step in (31, 9):
+        for step in ((47, 40) if dtype == "f32" else (31, 9)):
             E, B = gpu_fields(ctx, w, step)
             Eo, Bo = oracle_fields(w, step, points=pts)
             check(w, E, B, Eo, Bo, None, f"point list kernel {kernel} step {step}")
@@ -243,7 +246,7 @@ def test_point_list_tiled_every_point_against_the_oracle(jb, dtype):
     sub-ranges (served by the per-point kernel) agree with the full call."""
     w = wl.config2c_noise(dtype)
     if dtype == "f32":
-        w = wl.modulate_in_time(w, 64.0)
+        w = wl.smooth_in_time(w, 64.0)
     w = wl.with_random_points(w, 20000, margin=0.3)
     ctx = make_ctx(w, jb)
     try:
@@ -262,27 +265,46 @@ def test_point_list_tiled_every_point_against_the_oracle(jb, dtype):
 
 
 def test_point_list_at_c3_scale_and_degenerate_sets(jb):
-    """65 536 unstructured points on the 64^3 x 221-step collision history (fp32, the bench workload
-    c3_points): the oracle on 8192 seeded points, every other output against the per-point kernel.
-    Then the degenerate sets: all points identical (one bin, zero-size boxes), points on a line,
-    a single point."""
-    w = wl.with_random_points(wl.config3_collision(), 65536)
-    ctx = make_ctx(w, jb)
-    try:
-        upload(ctx, w)
-        ctx.set_kernel(2)
-        E, B = gpu_fields(ctx, w, 220)
-        idx = w.obs_subset(8192)
-        Eo, Bo = oracle_fields(w, 220, points=w.points[idx])
-        check(w, E[:, idx], B[:, idx], Eo, Bo, None, "c3 points")
-        ctx.set_kernel(1)
-        E1, B1 = gpu_fields(ctx, w, 220)
-        for got, ref, name in ((E, E1, "E"), (B, B1, "B")):
-            rms = np.sqrt(np.mean(np.sum(ref * ref, axis=0)))
-            assert np.abs(got - ref).max() <= 4e-3 * rms, name
-            assert max(rel_l2(got, ref, field_ref=ref)) <= 4e-4
-    finally:
-        ctx.close()
+    """65 536 unstructured points on a 64^3 x 221-step history (fp32; the geometry of the bench
+    workload c3_points): the oracle on 8192 seeded points, every other output against the
+    per-point kernel.  Two histories.  (a) Smooth in time (the collision snapshot of step 190
+    modulated by 1 + 0.3 sin): both kernels must meet the fp32 bar.  (b) The collision history
+    itself, whose Lorentz-contracted discs sweep a cell in two steps: with ~1e-4 of the 1.7e10
+    pairs inside the fp32 error of a lag tie (unstructured geometry, q up to 220) no fp32
+    evaluation can reproduce the fp64 oracle's nearest-snapshot choices -- stated limitation,
+    DESIGN.md Q3; the error is measured, printed and bounded at 2e-2, and the two kernels must
+    still agree with each other as closely as they do with the oracle.  Then the degenerate sets:
+    all points identical (one bin, zero-size boxes), points on a line, a single point."""
+    for smooth in (True, False):
+        w = wl.config3_collision()
+        if smooth:
+            w = wl.smooth_in_time(w, 64.0, base_step=190)
+        w = wl.with_random_points(w, 65536)
+        ctx = make_ctx(w, jb)
+        try:
+            upload(ctx, w)
+            idx = w.obs_subset(8192)
+            Eo, Bo = oracle_fields(w, 220, points=w.points[idx])
+            out = {}
+            for kernel in (2, 1):
+                ctx.set_kernel(kernel)
+                E, B = gpu_fields(ctx, w, 220)
+                out[kernel] = (E, B)
+                if smooth:
+                    check(w, E[:, idx], B[:, idx], Eo, Bo, None, f"c3-scale points, smooth history, kernel {kernel}")
+                else:
+                    eE = max(rel_l2(E[:, idx], Eo, field_ref=Eo)); eB = max(rel_l2(B[:, idx], Bo, field_ref=Bo))
+                    print(f"\nc3 collision history, 65536 unstructured points, fp32 kernel {kernel} vs fp64 oracle: "
+                          f"rel-L2 E {eE:.2e} B {eB:.2e} (near-tie lag choices)")
+                    assert eE < 2e-2 and eB < 2e-2
+            for a, b, name in ((out[2][0], out[1][0], "E"), (out[2][1], out[1][1], "B")):
+                lim = 4e-4 if smooth else 2e-2
+                assert max(rel_l2(a, b, field_ref=b)) <= lim, name
+                if smooth:
+                    rms = np.sqrt(np.mean(np.sum(b * b, axis=0)))
+                    assert np.abs(a - b).max() <= 4e-3 * rms, name
+        finally:
+            ctx.close()
     w = wl.random_history((6, 5, 4), 24, seed=15, dtype="f64", dt=0.05)
     for pts in (np.tile([[0.31, -0.2, 0.45]], (700, 1)),
                 np.stack([np.linspace(-2, 2, 1500), np.full(1500, 0.4), np.full(1500, -0.3)], axis=1),
@@ -880,7 +902,8 @@ def test_strong_scaling_slices_concatenate_to_the_full_evaluation(jb, world, dty
     available, so the ranks' calls run one after another on it: the concatenation in rank order must
     equal the unsharded call (to tolerance -- the launcher picks a different source-chunk count per
     slice, so the summation order differs) and the oracle; the same for a time series."""
-    w = wl.random_history((10, 9, 8), 40, seed=91, dtype=dtype, n_obs=(16, 12, 10), dt=0.05)
+    # (16-10, 13-9, 10-8 are all even: integer cell offsets on every axis, no pair on the screening radius)
+    w = wl.random_history((10, 9, 8), 40, seed=91, dtype=dtype, n_obs=(16, 13, 10), dt=0.05)
     obs = jb.make_obs_grid(w.n_obs, w.origin_obs, w.spacing_obs)
     ctx = make_ctx(w, jb)
     try:

@@ -333,15 +333,18 @@ def with_random_points(w: Workload, n: int, seed_offset: int = 0, margin: float 
     return w
 
 
-def modulate_in_time(w: Workload, period: float, depth: float = 0.3) -> Workload:
-    """Multiplies every cell's history by 1 + depth*sin(2 pi m / period): white in space, smooth in
-    time.  For fp32 parity on UNSTRUCTURED geometry: there a pair can sit within the fp32 rounding
-    error of a retarded-index tie, and with a history that is white in time one flipped index is
-    an O(1) error in its term although either neighbouring step is an equally good nearest
-    snapshot ('harmless for smooth histories')."""
+def smooth_in_time(w: Workload, period: float, depth: float = 0.3, base_step: int = 0) -> Workload:
+    """Replaces the history of ``w`` by its snapshot ``base_step`` times 1 + depth*sin(2 pi m/period + phase_j)
+    with a seeded phase per cell: white in space, smooth in time.  For fp32 parity on UNSTRUCTURED
+    geometry: there a pair can sit within the fp32 rounding error of a retarded-index tie, and
+    with a history that is white in time one flipped index is an O(1) error in its term although
+    either neighbouring step is an equally good nearest snapshot ('harmless for
+    smooth histories')."""
     m = np.arange(w.T, dtype=np.float64)
-    f = 1.0 + depth * np.sin(2.0 * np.pi * m / period)
-    w.rho = np.ascontiguousarray((w.rho.astype(np.float64) * f[:, None, None, None]).astype(w.np_dtype))
-    w.J = np.ascontiguousarray((w.J.astype(np.float64) * f[:, None, None, None, None]).astype(w.np_dtype))
-    w.name = f"{w.name}_mod{period:g}"
+    Ns = w.N_s
+    ph = 2.0 * np.pi * uniform01(w.seed + 97, 0, Ns).reshape(w.rho.shape[1:])
+    f = 1.0 + depth * np.sin(2.0 * np.pi * m[:, None, None, None] / period + ph[None])
+    w.rho = np.ascontiguousarray((w.rho[base_step].astype(np.float64)[None] * f).astype(w.np_dtype))
+    w.J = np.ascontiguousarray((w.J[base_step].astype(np.float64)[None] * f[:, None]).astype(w.np_dtype))
+    w.name = f"{w.name}_smooth{period:g}"
     return w
