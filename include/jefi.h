@@ -13,6 +13,13 @@
  *   m < 0 contributes zero (the paper's sources vanish before t0);
  *   cells with R < 0.5*min(dx,dy,dz) are skipped (coarse screening);
  *   dV = dx*dy*dz of the source grid.
+ *   Powers of c: the weights are exactly d/R^3, d/(c R^2), 1/(c^2 R) for E and 1/R^3, 1/(c R^2)
+ *   for B, with NO overall power of c on B (BASELINE.json north_star lists them so).  That is a
+ *   chosen convention, not a unit system: Heaviside-Lorentz, the paper's, would put
+ *   1/c on B.  The paper and every benchmark config have c = 1, where all conventions agree; a
+ *   caller with c != 1 who wants Heaviside-Lorentz B divides B_out by c.  An exact tie in the
+ *   retarded step, q = R/(c dt) a half-integer, rounds UP (Q3 says what finite
+ *   precision can and cannot decide there).
  *
  * Every step of that path runs in hand-written CUDA kernels; there is no CPU fallback and
  * no other backend.  All pointers named *_dev are DEVICE pointers of the context's dtype,

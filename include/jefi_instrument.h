@@ -24,6 +24,13 @@ int64_t     jefi_launch_count(const jefi_ctx* ctx);
  * (MEASURED_PEAKS.json carries no FP32/FP64 figure). */
 jefi_status jefi_measure_alu_peak(int device, jefi_dtype dtype, double* tflops);
 
+/* FP32 FFMA throughput by operand source on `device` (TFLOP/s, synchronous): accumulate
+ * instructions acc += v * w that read two fresh registers and one the operand-reuse cache serves,
+ * and ones that read three fresh registers.  jefi_measure_alu_peak's chain takes its other two
+ * operands from the constant bank.  bench.py prints all three beside the series workloads: the
+ * register file, not the FMA pipe, bounds the time-blocked kernel. */
+jefi_status jefi_measure_ffma_operand_rates(int device, double* two_fresh_tflops, double* three_fresh_tflops);
+
 /* Retarded lag k (Eq. (6): the stored step is m = step - k) that kernel `which`
  * computes for n_pairs explicit (observation point, source cell) pairs:
  * obs_index_dev[i] = linear index into the observation set, cell_index_dev[i] = linear source

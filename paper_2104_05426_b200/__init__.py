@@ -27,7 +27,7 @@ EXPORTS = (                                   # include/jefi.h: the product ABI
     "jefi_append_step", "jefi_append_step_host", "jefi_fields_series", "jefi_fields_series_host",
 )
 INSTRUMENT_EXPORTS = (                        # include/jefi_instrument.h: bench / test instrumentation
-    "jefi_launch_count", "jefi_measure_alu_peak", "jefi_debug_pair_lags", "jefi_debug_launch_limits",
+    "jefi_launch_count", "jefi_measure_alu_peak", "jefi_measure_ffma_operand_rates", "jefi_debug_pair_lags", "jefi_debug_launch_limits",
 )
 
 
@@ -84,6 +84,7 @@ _lib.jefi_flops_per_pair.argtypes = []
 _lib.jefi_measure_alu_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
 _lib.jefi_shard_obs.argtypes = [C.POINTER(jefi_obs_desc), C.c_int32, C.c_int32, C.POINTER(C.c_int64),
                                 C.POINTER(C.c_int64)]
+_lib.jefi_measure_ffma_operand_rates.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
 _lib.jefi_debug_pair_lags.argtypes = [_P, C.c_int32, C.c_int64, _P, _P, _P, _P]
 _lib.jefi_debug_launch_limits.argtypes = [_P, C.c_int64, C.c_int64]
 for _n in EXPORTS + INSTRUMENT_EXPORTS:
@@ -214,6 +215,15 @@ def jefi_measure_alu_peak(device: int, dtype: int) -> float:
     if st != JEFI_OK:
         raise JefiError(st, "jefi_measure_alu_peak")
     return v.value
+
+
+def jefi_measure_ffma_operand_rates(device: int):
+    """(two fresh registers + one reused, three fresh registers) FFMA rates in TFLOP/s."""
+    a, b = C.c_double(), C.c_double()
+    st = _lib.jefi_measure_ffma_operand_rates(int(device), C.byref(a), C.byref(b))
+    if st != JEFI_OK:
+        raise JefiError(st, "jefi_measure_ffma_operand_rates")
+    return a.value, b.value
 
 
 def jefi_debug_pair_lags(ctx, which: int, n_pairs: int, obs_index_dev, cell_index_dev, lag_out_dev, stream=None):

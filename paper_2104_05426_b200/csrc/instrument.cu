@@ -51,6 +51,58 @@ double run_chain(int sm_count)
     return best;
 }
 
+// FP32 FFMA rate as a function of where the operands come from (what bounds
+// the time-blocked kernel once the shared-memory gather is relieved).  MODE 0: 64 accumulators,
+// acc += v[j % 8] * w -- two fresh register reads (accumulator, value) and one the operand-reuse
+// cache serves (w); MODE 1: acc += v[a] * u[b] with all three registers fresh.
+template <int MODE>
+__global__ void __launch_bounds__(256)
+ffma_operand_kernel(float* out, const float* in, int iters)
+{
+    float acc[64], v[32], u[32];
+    for (int i = 0; i < 64; ++i) acc[i] = threadIdx.x + i;
+    for (int i = 0; i < 32; ++i) { v[i] = in[i + threadIdx.x]; u[i] = in[i + 64 + threadIdx.x]; }
+    float w = in[100 + threadIdx.x];
+    for (int it = 0; it < iters; ++it) {
+        if (MODE == 0) {
+#pragma unroll
+            for (int j = 0; j < 64; ++j) acc[j] = fmaf(v[j % 8], w, acc[j]);
+            w += 1e-9f;
+        } else {
+#pragma unroll
+            for (int j = 0; j < 64; ++j) acc[j] = fmaf(v[j % 32], u[(j * 7 + 3) % 32], acc[j]);
+        }
+    }
+    float s = 0;
+    for (int i = 0; i < 64; ++i) s += acc[i];
+    if (s == -12345.678f) out[0] = s;
+}
+
+template <int MODE>
+double run_operand(int sm_count)
+{
+    float *out = nullptr, *in = nullptr;
+    if (cudaMalloc(&out, 64) != cudaSuccess || cudaMalloc(&in, 4096) != cudaSuccess) return -1.0;
+    cudaMemset(in, 0, 4096);
+    const int iters = 2048, blocks = sm_count * 8;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    double best = -1.0;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0);
+        ffma_operand_kernel<MODE><<<blocks, 256>>>(out, in, iters);
+        cudaEventRecord(e1);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { best = -1.0; break; }
+        float ms = 0;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double tf = 2.0 * 64.0 * iters * 256.0 * blocks / (ms * 1e-3) * 1e-12;
+        if (rep > 0 && tf > best) best = tf;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(out); cudaFree(in);
+    return best;
+}
+
 // ------------------------------------------------------------------ lag dump
 struct LagArgs {
     int nsx, nsy, nox, noy;
@@ -112,6 +164,18 @@ jefi_status jefi_measure_alu_peak(int device, jefi_dtype dtype, double* tflops)
                                        : jefi::run_chain<double>(prop.multiProcessorCount);
     if (v < 0) { cudaGetLastError(); return JEFI_ERR_CUDA; }
     *tflops = v;
+    return JEFI_OK;
+}
+
+jefi_status jefi_measure_ffma_operand_rates(int device, double* two_fresh_tflops, double* three_fresh_tflops)
+{
+    if (!two_fresh_tflops || !three_fresh_tflops || device < 0) return JEFI_ERR_INVALID_ARG;
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return JEFI_ERR_CUDA; }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaGetLastError(); return JEFI_ERR_CUDA; }
+    const double a = jefi::run_operand<0>(prop.multiProcessorCount), b = jefi::run_operand<1>(prop.multiProcessorCount);
+    if (a < 0 || b < 0) { cudaGetLastError(); return JEFI_ERR_CUDA; }
+    *two_fresh_tflops = a; *three_fresh_tflops = b;
     return JEFI_OK;
 }
 

@@ -5,13 +5,17 @@
 // on the evaluation step n.  So a thread computes them ONCE per pair and then walks NS output
 // steps n0 .. n0+NS-1, whose retarded steps m_i = n0 + i - k are CONSECUTIVE stored snapshots.
 //
-// What that buys on the binding unit.  The one-step kernel (pairwise_tiled.cu) gathers a 32-byte
-// record {rho, rho_dot, J, J_dot} per pair through the shared-memory pipe, which ncu shows 89 %
-// busy.  Here the history is kept as RAW 16-byte records {rho, Jx/c, Jy/c, Jz/c} per (cell, step)
-// ("series layout", built from the packed history by series_layout_kernel below), a thread loads
-// the NS+2 consecutive slots m_0-1 .. m_{NS-1}+1 and forms the time differences in registers:
-// 16 (NS+2)/NS lane-bytes per (pair, step) -- 20 B at NS = 8 instead of 32 -- and the geometry
-// (7 FMA-pipe instructions, the MUFU, the address) is paid once per NS steps.
+// What that buys.  The one-step kernel (pairwise_tiled.cu) gathers a 32-byte record {rho, rho_dot,
+// J, J_dot} per pair through the shared-memory pipe, which ncu shows 89 % busy.  Here the history
+// is kept as RAW 16-byte records {rho, Jx/c, Jy/c, Jz/c} per (cell, step) ("series layout", built
+// from the packed history by series_layout_kernel below), a thread loads the NS+2 consecutive
+// slots m_0-1 .. m_{NS-1}+1 and forms the time differences in registers: 16 (NS+2)/NS lane-bytes
+// per (pair, step) -- 21.3 B at NS = 6 instead of 32 -- and the geometry (7 FMA-pipe
+// instructions, the MUFU, the address) is paid once per NS steps.  With the gather relieved
+// (shared pipe 54 % busy) the bound moves to the register file: an FFMA that reads two fresh
+// registers and one reused one sustains 89 % of the FMA-pipe rate on this chip, three fresh ones
+// 57 %, and this loop's 4 FADD + 14 FFMA per step 72 % on its own, 4.3 pair-steps per clock per SM
+// with its loads (micro-benchmarks); the kernel reaches 3.7.
 //
 // Arithmetic per (pair, step), pre-scaled variables as in prepass.cu (E = sum d (rho/R^3 +
 // rho_dot'/R^2) - J_dot''/R, B = c sum (J'/R^3 + J_dot''/R^2) x d with rho_dot' = rho_dot/c,
