@@ -44,6 +44,8 @@ list_bbox_kernel(const T* __restrict__ pts, long long n, unsigned long long* __r
     for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256)
         for (int a = 0; a < 3; ++a) {
             const double v = (double)pts[3 * i + a];
+            // a NaN or Inf position makes the box infinite: build_tiles_T reports it
+            if (!isfinite(v)) { lo[a] = -INFINITY; hi[a] = INFINITY; continue; }
             lo[a] = v < lo[a] ? v : lo[a]; hi[a] = v > hi[a] ? v : hi[a];
         }
     for (int a = 0; a < 3; ++a) {
