@@ -121,6 +121,18 @@ def test_series_matches_single_step_calls_and_errors(jb):
         with pytest.raises(jb.JefiError) as e:
             ctx.fields_series(10, 11, E, torch.empty_like(E))
         assert e.value.status == jb.JEFI_ERR_TIME_RANGE
+        # host-buffer entry point: the same values, through the context's staging (grown on demand)
+        for begin, count in ((4, 16), (0, 20), (7, 3)):
+            Eh = torch.empty((count, 3, w.N_o), dtype=torch.float32).pin_memory()
+            Bh = torch.empty_like(Eh).pin_memory()
+            ctx.fields_series_host(begin, count, Eh, Bh)
+            torch.cuda.synchronize()
+            Ed, Bd = gpu_fields_series(ctx, w, begin, count)
+            np.testing.assert_array_equal(Eh.numpy().astype(np.float64), Ed)
+            np.testing.assert_array_equal(Bh.numpy().astype(np.float64), Bd)
+        with pytest.raises(jb.JefiError) as e:
+            jb.jefi_fields_series_host(ctx.ctx, 0, 4, 0, w.N_o, None, Bh)
+        assert e.value.status == jb.JEFI_ERR_INVALID_ARG
         # after an append the series layout is rebuilt
         ctx.append_step(torch.from_numpy(w.rho[3]).cuda(), torch.from_numpy(w.J[3]).cuda())
         Es2, _ = gpu_fields_series(ctx, w, 4, 16)
