@@ -127,6 +127,40 @@ def test_null_context_is_an_error_not_a_crash(jb):
     assert lib.jefi_measure_alu_peak(0, 0, None) == jb.JEFI_ERR_INVALID_ARG
 
 
+def test_series_and_instrument_entry_points_reject_null_arguments(jb):
+    lib = C.CDLL(str(jb.LIB_PATH))
+    P = C.c_void_p
+    lib.jefi_fields_series.argtypes = [P, C.c_int32, C.c_int32, C.c_int64, C.c_int64, P, P, P]
+    lib.jefi_fields_series_host.argtypes = [P, C.c_int32, C.c_int32, C.c_int64, C.c_int64, P, P, P]
+    assert lib.jefi_fields_series(None, 0, 4, 0, 0, None, None, None) == jb.JEFI_ERR_INVALID_ARG
+    assert lib.jefi_fields_series_host(None, 0, 4, 0, 0, None, None, None) == jb.JEFI_ERR_INVALID_ARG
+    lib.jefi_debug_pair_lags.argtypes = [P, C.c_int32, C.c_int64, P, P, P, P]
+    assert lib.jefi_debug_pair_lags(None, 2, 1, None, None, None, None) == jb.JEFI_ERR_INVALID_ARG
+    lib.jefi_debug_launch_limits.argtypes = [P, C.c_int64, C.c_int64]
+    assert lib.jefi_debug_launch_limits(None, 1, 1) == jb.JEFI_ERR_INVALID_ARG
+    lib.jefi_measure_ffma_operand_rates.argtypes = [C.c_int, P, P]
+    assert lib.jefi_measure_ffma_operand_rates(0, None, None) == jb.JEFI_ERR_INVALID_ARG
+    lib.jefi_launch_count.argtypes = [P]
+    lib.jefi_launch_count.restype = C.c_int64
+    assert lib.jefi_launch_count(None) == 0
+    lib.jefi_set_kernel.argtypes = [P, C.c_int32]
+    assert lib.jefi_set_kernel(None, 3) == jb.JEFI_ERR_INVALID_ARG
+
+
+def test_create_rejects_a_point_list_without_positions(jb):
+    src, obs, tm = _descs(jb)
+    pts = jb.jefi_obs_desc()
+    pts.kind, pts.npoints, pts.points_dev = 1, 100, None
+    pts.grid = jb.make_grid((1, 1, 1), (0, 0, 0), (1, 1, 1))
+    with pytest.raises(jb.JefiError) as e:
+        jb.jefi_create(src, pts, tm, jb.JEFI_F32, 0)
+    assert e.value.status == jb.JEFI_ERR_INVALID_ARG
+    pts.npoints = -1
+    with pytest.raises(jb.JefiError) as e:
+        jb.jefi_create(src, pts, tm, jb.JEFI_F32, 0)
+    assert e.value.status == jb.JEFI_ERR_INVALID_ARG
+
+
 def test_product_does_not_import_the_oracle():
     """The product path must never route through oracle/ (or workloads' arithmetic-free data)."""
     pkg = os.path.join(ROOT, "paper_2104_05426_b200")
