@@ -126,7 +126,8 @@ jefi_status jefi_upload_history_host(jefi_ctx* ctx, const void* rho_host, const 
  * one included -- keeps the value it had.  The packed history therefore equals, record for
  * record and bit for bit, the last nsteps records of a pre-pass over the (nsteps+1)-step raw
  * history [old steps..., new step].  Needs a prior jefi_upload_history (JEFI_ERR_NO_HISTORY).
- * One kernel on `stream`: an in-place shift of the packed history (read + write of it once). */
+ * One kernel on `stream`.  The stored steps of a cell form a ring inside the context, so the
+ * call writes two records per cell -- O(N_s) bytes, whatever the history length. */
 jefi_status jefi_append_step(jefi_ctx* ctx, const void* rho_new_dev, const void* J_new_dev,
                              jefi_stream stream);
 

@@ -202,6 +202,7 @@ jefi_status jefi_upload_history(jefi_ctx* ctx, const void* rho_dev, const void* 
     if (!rho_dev || !J_dev) { set_err(ctx, "null history pointer", cudaSuccess); return JEFI_ERR_INVALID_ARG; }
     cudaError_t e = cudaSetDevice(ctx->device);
     if (e != cudaSuccess) return cuda_fail(ctx, "cudaSetDevice", e);
+    ctx->P.origin = 0;                     // the pre-pass writes packed step p at slot p
     int n = jefi::launch_prepass(ctx->P, ctx->dtype, rho_dev, J_dev, ctx->hist, (cudaStream_t)stream);
     if (n < 0) return cuda_fail(ctx, "pre-pass launch", cudaGetLastError());
     ctx->launches += n;
@@ -244,6 +245,7 @@ jefi_status jefi_append_step(jefi_ctx* ctx, const void* rho_new_dev, const void*
                                 (cudaStream_t)stream);
     if (n < 0) return cuda_fail(ctx, "append launch", cudaGetLastError());
     ctx->launches += n;
+    ctx->P.origin = (ctx->P.origin + 1) % ctx->P.T;      // the ring advances: packed step p now sits one slot on
     ctx->series_valid = false;
     ctx->t0 += ctx->P.dt;
     return JEFI_OK;

@@ -22,6 +22,7 @@ struct Params {
     long long Ns;           // source cells
     int     T;              // stored steps
     int     Tp;             // T + 1: packed steps p = m + 1, p = 0 is the all-zero record
+    int     origin;         // ring origin of the packed history (tiled_common.cuh ring_slot)
     double  dt, c;
     int     deriv_mode;
 };

@@ -172,7 +172,7 @@ struct ListArgs {
     int nsx, nsy, nsz;
     double shx, shy, shz, sox, soy, soz;
     double rcut2, inv_cdt;
-    int Tp, n1;
+    int Tp, n1, origin;
     long long n_points, obs_count;            // the whole list is evaluated (obs_begin = 0)
     long long cells_per_chunk, Ns;
     int wcap_rt, chunk_base, accumulate, flush_stages;
@@ -230,9 +230,11 @@ fields_list_kernel(const uint4* __restrict__ hist, double* __restrict__ partial,
                 slow = dmin2 <= a.rcut2 * 1.001;
                 int p_hi = a.n1 - kmin;
                 p_hi = p_hi > a.Tp - 1 ? a.Tp - 1 : p_hi;
-                nz = p_lo < 0 ? -p_lo : 0;
+                // slots for p <= 0 (the zero record and everything before it) are zero-filled here;
+                // stored steps p >= 1 are copied from the ring
+                nz = p_lo < 1 ? 1 - p_lo : 0;
                 nz = nz > span ? span : nz;
-                p_src = p_lo < 0 ? 0 : p_lo;
+                p_src = p_lo < 1 ? 1 : p_lo;
                 cnt = p_hi >= p_src ? p_hi - p_src + 1 : 0;
                 cnt = cnt > span - nz ? span - nz : cnt;
                 row0 = data0 + (unsigned)s * (unsigned)a.stage_bytes + (unsigned)lane * (unsigned)U * unit_off;
@@ -253,10 +255,17 @@ fields_list_kernel(const uint4* __restrict__ hist, double* __restrict__ partial,
                 const unsigned bytes = (unsigned)cnt * 16u;
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 mbar_arrive_expect_tx(bar, (unsigned)U * bytes);
-                const uint4* src = hist + ((size_t)j * U) * a.Tp + p_src;
+                // the window is contiguous in p; in the ring it is one piece, or two when it wraps
+                const int slot1 = ring_slot(p_src, a.origin, a.Tp - 1);
+                const int len1 = cnt < a.Tp - slot1 ? cnt : a.Tp - slot1;
+                const uint4* src = hist + ((size_t)j * U) * a.Tp;
 #pragma unroll
-                for (int u = 0; u < U; ++u)
-                    bulk_g2s(row0 + u * unit_off + (unsigned)nz * 16u, src + (size_t)u * a.Tp, bytes, bar);
+                for (int u = 0; u < U; ++u) {
+                    const unsigned dst = row0 + u * unit_off + (unsigned)nz * 16u;
+                    bulk_g2s(dst, src + (size_t)u * a.Tp + slot1, (unsigned)len1 * 16u, bar);
+                    if (len1 < cnt)
+                        bulk_g2s(dst + (unsigned)len1 * 16u, src + (size_t)u * a.Tp + 1, (unsigned)(cnt - len1) * 16u, bar);
+                }
             } else {
                 mbar_arrive(bar);
             }
@@ -362,7 +371,7 @@ int launch_list_cap(const Params& P, jefi_dtype dt, const void* hist, const Fiel
     hmin = hmin < P.sh[2] ? hmin : P.sh[2];
     a.rcut2 = 0.25 * hmin * hmin;
     a.inv_cdt = 1.0 / (P.c * P.dt);
-    a.Tp = P.Tp; a.n1 = L.step + 1;
+    a.Tp = P.Tp; a.n1 = L.step + 1; a.origin = P.origin;
     a.n_points = P.n_obs; a.obs_count = L.obs_count;
     a.Ns = P.Ns;
     a.points = P.obs_points; a.perm = pt.perm; a.boxes = pt.boxes;

@@ -39,7 +39,7 @@ struct PointArgs {
     double sox, soy, soz;       // source origin (for explicit point lists)
     double rcut2, inv_cdt;
     long long Ns, obs_begin, obs_count;
-    int Tp, n1;                 // n1 = step + 1
+    int Tp, n1, origin;         // n1 = step + 1; ring origin of the packed history
     int obs_kind;
     const void* points;
     long long cells_per_chunk;
@@ -89,7 +89,7 @@ fields_point_kernel(const T* __restrict__ hist, double* __restrict__ partial, Po
             point_geo<T>(ox, sx, shx, ryz, rcut2, inv_cdt, dx, rinv, k);
             int p = a.n1 - k;
             p = p < 0 ? 0 : p;
-            const Rec<T> h = load_rec(hist, j, a.Tp, p);      // rho, rho', Jx, Jy, Jz, Jx', Jy', Jz'
+            const Rec<T> h = load_rec(hist, j, a.Tp, ring_slot(p, a.origin, a.Tp - 1));      // rho, rho', Jx, Jy, Jz, Jx', Jy', Jz'
             const T r2 = rinv * rinv;
             const T s  = (h.v[0] * rinv + h.v[1]) * r2;
             const T ux = (h.v[2] * rinv + h.v[5]) * r2;
@@ -170,7 +170,7 @@ int launch_fields_point(const Params& P, jefi_dtype dt, const void* hist, const 
     a.rcut2 = 0.25 * hmin * hmin;
     a.inv_cdt = 1.0 / (P.c * P.dt);
     a.Ns = P.Ns; a.obs_begin = L.obs_begin; a.obs_count = L.obs_count;
-    a.Tp = P.Tp; a.n1 = L.step + 1;
+    a.Tp = P.Tp; a.n1 = L.step + 1; a.origin = P.origin;
     a.obs_kind = P.obs_kind; a.points = P.obs_points;
 
     const long long blocks = (L.obs_count + kPointThreads - 1) / kPointThreads;

@@ -69,11 +69,11 @@ struct SeriesArgs {
 // One thread per (cell, slot); reads and writes are coalesced along the slot index (both layouts are
 // [cell][unit][step]).  HBM-bound: 32 B read + 16 B written per record (fp32).
 template <typename T>
-__device__ __forceinline__ void packed_values(const T* __restrict__ packed, long long j, int Tp, int m, T (&f)[4])
+__device__ __forceinline__ void packed_values(const T* __restrict__ packed, long long j, int Tp, int origin, int m, T (&f)[4])
 {
     // values rho, Jx', Jy', Jz' of stored step m (packed step m + 1)
     constexpr int VPU = 16 / sizeof(T), U = 8 / VPU;
-    const long long base = (j * U) * (long long)Tp + (m + 1);
+    const long long base = (j * U) * (long long)Tp + ring_slot(m + 1, origin, Tp - 1);
     constexpr int idx[4] = {0, 2, 3, 4};
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
@@ -85,7 +85,7 @@ __device__ __forceinline__ void packed_values(const T* __restrict__ packed, long
 template <typename T>
 __global__ void __launch_bounds__(256)
 series_layout_kernel(const T* __restrict__ packed, T* __restrict__ series, long long Ns, int Tsteps, int Tp, int Tq,
-                     int backward)
+                     int backward, int origin)
 {
     constexpr int VPU = 16 / sizeof(T), U = 4 / VPU;         // series units per record: 1 (fp32), 2 (fp64)
     const long long t = (long long)blockIdx.x * 256 + threadIdx.x;
@@ -95,14 +95,14 @@ series_layout_kernel(const T* __restrict__ packed, T* __restrict__ series, long 
     T f[4] = {0, 0, 0, 0};
     const int m = p - 2;
     if (m >= 0 && m < Tsteps) {
-        packed_values<T>(packed, j, Tp, m, f);
+        packed_values<T>(packed, j, Tp, origin, m, f);
     } else if (!backward && (m == -1 || m == Tsteps)) {
         // ghost: 2 f[end] - f[next to end] (one rounding); T = 1: f[0]
         const int e = m == -1 ? 0 : Tsteps - 1, e2 = m == -1 ? 1 : Tsteps - 2;
         T a[4], b[4];
-        packed_values<T>(packed, j, Tp, e, a);
+        packed_values<T>(packed, j, Tp, origin, e, a);
         if (Tsteps >= 2) {
-            packed_values<T>(packed, j, Tp, e2, b);
+            packed_values<T>(packed, j, Tp, origin, e2, b);
 #pragma unroll
             for (int q = 0; q < 4; ++q) f[q] = fma_t<T>(T(2), a[q], -b[q]);
         } else {
@@ -599,10 +599,10 @@ int launch_series_layout(const Params& P, jefi_dtype dt, const void* packed, voi
     const unsigned blocks = (unsigned)((total + 255) / 256);
     if (dt == JEFI_F32)
         series_layout_kernel<float><<<blocks, 256, 0, stream>>>((const float*)packed, (float*)series, P.Ns, P.T, P.Tp,
-                                                                 Tq, P.deriv_mode);
+                                                                 Tq, P.deriv_mode, P.origin);
     else
         series_layout_kernel<double><<<blocks, 256, 0, stream>>>((const double*)packed, (double*)series, P.Ns, P.T,
-                                                                  P.Tp, Tq, P.deriv_mode);
+                                                                  P.Tp, Tq, P.deriv_mode, P.origin);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 

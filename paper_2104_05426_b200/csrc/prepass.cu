@@ -16,7 +16,7 @@
 // HBM-bound: 16 B read + 32 B written per record (fp32); the transpose from the cell-fastest
 // input to the time-fastest output goes through a padded shared-memory tile so that both the
 // global reads (lanes along cells) and the global writes (lanes along steps) are coalesced.
-#include "jefi_internal.h"
+#include "tiled_common.cuh"
 
 namespace jefi {
 namespace {
@@ -114,13 +114,14 @@ prepass_march_kernel(const T* __restrict__ rho, const T* __restrict__ J, Unit<T>
 
 // ---------------------------------------------------------------------------------------------
 // Sliding window (the history holds lts = ceil(d_m/dt) snapshots, i.e. as far back
-// as the longest delay; it stays on the GPU between calls).  append_kernel drops
-// the oldest stored step, shifts every [cell][unit] row by one slot in place, writes the record
-// of the new newest step (one-sided derivative (f_new - f_prev)/dt) and, in centred mode,
-// re-differences the previous newest step now that its successor exists:
-// (f_new - f_prev2)/(2 dt).  `last` holds the raw values of the two newest steps
-// ([2][4][N_s]: step T-2, step T-1; component 0 = rho, 1..3 = J) so that both records are
-// bit-identical to what the pre-pass makes of the same raw history.  One warp per cell.
+// as the longest delay; it stays on the GPU between calls).  The stored steps of a
+// row form a ring (tiled_common.cuh ring_slot): append_kernel overwrites the slot of the OLDEST
+// step with the record of the new newest one (one-sided derivative (f_new - f_prev)/dt) and,
+// in centred mode, re-differences the previous newest step now that its successor exists:
+// (f_new - f_prev2)/(2 dt); the host then advances the ring origin by one.  Two records per
+// (cell, unit) are written, whatever the history length.  `last` holds the raw values of the
+// two newest steps ([2][4][N_s]: step T-2, step T-1; component 0 = rho, 1..3 = J) so that both
+// records are bit-identical to what the pre-pass makes of the same raw history.  One thread per cell.
 template <typename T>
 __device__ __forceinline__ void pack_record(const T (&f)[4], const T (&d)[4], T inv_c, T (&val)[8])
 {
@@ -131,11 +132,11 @@ __device__ __forceinline__ void pack_record(const T (&f)[4], const T (&d)[4], T 
 
 template <typename T>
 __global__ void __launch_bounds__(kThreads)
-append_kernel(const T* __restrict__ rho_new, const T* __restrict__ J_new, T* last, Unit<T>* hist, long long Ns, int Tsteps, int Tp, T inv_dt, T inv_c, int deriv_mode)
+append_kernel(const T* __restrict__ rho_new, const T* __restrict__ J_new, T* last, Unit<T>* hist, long long Ns, int Tsteps,
+              int Tp, int origin, T inv_dt, T inv_c, int deriv_mode)
 {
     constexpr int U = sizeof(T) == 4 ? 2 : 4, VPU = 8 / U;
-    const long long j = (long long)blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5);
-    const int lane = threadIdx.x & 31;
+    const long long j = (long long)blockIdx.x * kThreads + threadIdx.x;
     if (j >= Ns) return;
 
     T fn[4], fp[4], fq[4], dn[4], dp[4];
@@ -151,38 +152,27 @@ append_kernel(const T* __restrict__ rho_new, const T* __restrict__ J_new, T* las
     pack_record<T>(fn, dn, inv_c, vn);
     pack_record<T>(fp, dp, inv_c, vp);
     const bool redo_prev = deriv_mode == 0 && Tsteps >= 2;
-
+    // `origin` is the ring origin BEFORE this append: the oldest step (p = 1) sits at slot
+    // 1 + origin and becomes the new newest one; the previous newest (p = T) sits one slot before it
+    const int slot_new = 1 + origin;
+    const int slot_prev = 1 + (origin + Tsteps - 1) % Tsteps;
 #pragma unroll
     for (int u = 0; u < U; ++u) {
         Unit<T>* row = hist + (j * U + u) * Tp;
-        // slots 2..T move to 1..T-1 (slot 0 is the all-zero record); ascending, one warp per row:
-        // a chunk is read completely before it is written, and the next chunk reads beyond it
-        const int last_dst = redo_prev ? Tsteps - 2 : Tsteps - 1;
-        for (int p0 = 1; p0 <= last_dst; p0 += 32) {
-            const int p = p0 + lane;
-            Unit<T> v;
-            if (p <= last_dst) v = row[p + 1];
-            __syncwarp();
-            if (p <= last_dst) row[p] = v;
-        }
-        if (lane == 0) {
-            Unit<T> q;
+        Unit<T> q;
 #pragma unroll
-            for (int e = 0; e < VPU; ++e) q.v[e] = vn[u * VPU + e];
-            row[Tsteps] = q;
-            if (redo_prev) {
+        for (int e = 0; e < VPU; ++e) q.v[e] = vn[u * VPU + e];
+        row[slot_new] = q;
+        if (redo_prev) {
 #pragma unroll
-                for (int e = 0; e < VPU; ++e) q.v[e] = vp[u * VPU + e];
-                row[Tsteps - 1] = q;
-            }
+            for (int e = 0; e < VPU; ++e) q.v[e] = vp[u * VPU + e];
+            row[slot_prev] = q;
         }
     }
-    if (lane == 0) {
 #pragma unroll
-        for (int comp = 0; comp < 4; ++comp) {
-            last[(long long)(0 * 4 + comp) * Ns + j] = fp[comp];
-            last[(long long)(1 * 4 + comp) * Ns + j] = fn[comp];
-        }
+    for (int comp = 0; comp < 4; ++comp) {
+        last[(long long)(0 * 4 + comp) * Ns + j] = fp[comp];
+        last[(long long)(1 * 4 + comp) * Ns + j] = fn[comp];
     }
 }
 
@@ -223,14 +213,14 @@ int launch_prepass(const Params& P, jefi_dtype dt, const void* rho, const void* 
 int launch_append(const Params& P, jefi_dtype dt, const void* rho_new, const void* J_new, void* last,
                   void* hist, cudaStream_t stream)
 {
-    const unsigned blocks = (unsigned)((P.Ns + kThreads / 32 - 1) / (kThreads / 32));
+    const unsigned blocks = (unsigned)((P.Ns + kThreads - 1) / kThreads);
     if (dt == JEFI_F32)
         append_kernel<float><<<blocks, kThreads, 0, stream>>>(
-            (const float*)rho_new, (const float*)J_new, (float*)last, (Unit<float>*)hist, P.Ns, P.T, P.Tp,
+            (const float*)rho_new, (const float*)J_new, (float*)last, (Unit<float>*)hist, P.Ns, P.T, P.Tp, P.origin,
             (float)(1.0 / P.dt), (float)(1.0 / P.c), P.deriv_mode);
     else
         append_kernel<double><<<blocks, kThreads, 0, stream>>>(
-            (const double*)rho_new, (const double*)J_new, (double*)last, (Unit<double>*)hist, P.Ns, P.T, P.Tp,
+            (const double*)rho_new, (const double*)J_new, (double*)last, (Unit<double>*)hist, P.Ns, P.T, P.Tp, P.origin,
             1.0 / P.dt, 1.0 / P.c, P.deriv_mode);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }

@@ -449,6 +449,44 @@ def test_append_step_slides_the_window(jb, dtype, c, deriv_mode):
         ctx.close()
 
 
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_append_step_ring_wraps_around_several_times(jb, dtype):
+    """47 appends on a 20-step history: the ring origin goes round twice and then some, so the
+    windows the producers copy wrap at every position; after each of the last appends the three
+    kernels (per-point, tiled, time-blocked series) equal a fresh upload of the last 20 steps --
+    bit for bit for the one-step kernels -- and the oracle on the whole raw history."""
+    import torch
+    T, A = 20, 47
+    full = wl.random_history((6, 5, 4), T + A, seed=45, dtype=dtype, n_obs=(9, 8, 5), dt=0.05)
+    first = _window(full, 0, T)
+    ctx = make_ctx(first, jb)
+    try:
+        upload(ctx, first)
+        for a in range(A):
+            ctx.append_step(torch.from_numpy(full.rho[T + a]).cuda(), torch.from_numpy(full.J[T + a]).cuda())
+            if a < A - 3:
+                continue
+            fresh_w = _window(full, a + 1, T)
+            fresh = make_ctx(fresh_w, jb)
+            try:
+                upload(fresh, fresh_w)
+                for kernel in KERNELS:
+                    ctx.set_kernel(kernel); fresh.set_kernel(kernel)
+                    E1, B1 = gpu_fields(ctx, first, T - 1)
+                    E2, B2 = gpu_fields(fresh, fresh_w, T - 1)
+                    np.testing.assert_array_equal(E1, E2)
+                    np.testing.assert_array_equal(B1, B2)
+                Eo, Bo = oracle_fields(full, T + a, None)
+                check(full, E1, B1, Eo, Bo, None, f"ring after {a + 1} appends")
+                ctx.set_kernel(3)
+                Es, Bs = gpu_fields_series(ctx, first, T - 6, 6)
+                check(full, Es[5], Bs[5], Eo, Bo, None, f"ring after {a + 1} appends, series")
+            finally:
+                fresh.close()
+    finally:
+        ctx.close()
+
+
 def test_append_step_single_stored_step_and_errors(jb):
     import torch
     w = wl.random_history((3, 3, 2), 3, seed=43, dtype="f64", n_obs=(2, 2, 2), spacing_obs=(0.01, 0.01, 0.01),
