@@ -242,7 +242,7 @@ def test_explicit_point_list_matches_oracle(jb, dtype, kernel):
 def test_point_list_tiled_every_point_against_the_oracle(jb, dtype):
     """20 000 unstructured points (40 / 79 tiles, the last ragged) in and around the 32^3 source grid
     of configs[1]: EVERY output of the tiled list kernel against the oracle; the outputs come
-    back in the caller's order although the kernel works through a Morton-sorted permutation;
+    back in the caller's order although the kernel works through a Hilbert-sorted permutation;
     sub-ranges (served by the per-point kernel) agree with the full call."""
     w = wl.config2c_noise(dtype)
     if dtype == "f32":
@@ -483,6 +483,30 @@ def test_append_step_ring_wraps_around_several_times(jb, dtype):
                 check(full, Es[5], Bs[5], Eo, Bo, None, f"ring after {a + 1} appends, series")
             finally:
                 fresh.close()
+    finally:
+        ctx.close()
+
+
+def test_append_step_with_a_point_list(jb):
+    """The ring history under the tiled list kernel and the per-point kernel: 700 unstructured
+    points, 9 appends on a 16-step history (fp64, white noise), each against the oracle."""
+    import torch
+    T, A = 16, 9
+    # (dt = 0.1: the longest lag is 12 < T-1, so neither a dropped step nor the oldest record is read)
+    full = wl.random_history((6, 5, 4), T + A, seed=47, dtype="f64", dt=0.1)
+    u = wl.uniform01(4747, 0, 3 * 700).reshape(700, 3)
+    pts = (u - 0.5) * np.array([1.0, 0.9, 0.8])
+    first = _window(full, 0, T)
+    ctx = make_ctx(first, jb, points=pts)
+    try:
+        upload(ctx, first)
+        for a in range(A):
+            ctx.append_step(torch.from_numpy(full.rho[T + a]).cuda(), torch.from_numpy(full.J[T + a]).cuda())
+            Eo, Bo = oracle_fields(full, T + a, points=pts)
+            for kernel in (2, 1):
+                ctx.set_kernel(kernel)
+                E, B = gpu_fields(ctx, first, T - 1)
+                check(full, E, B, Eo, Bo, None, f"list after {a + 1} appends, kernel {kernel}")
     finally:
         ctx.close()
 
