@@ -994,3 +994,37 @@ def test_strong_scaling_slices_concatenate_to_the_full_evaluation(jb, world, dty
             check(w, Esc[k], Bsc[k], Eo, Bo, None, f"strong x{world} {dtype} series step {30 + k}")
     finally:
         ctx.close()
+
+
+@pytest.mark.parametrize("world", [2, 5])
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_source_slabs_sum_to_the_full_evaluation(jb, world, dtype):
+    """bench.py --scaling strong --split src, the other decomposition of PAPER.md Fig. 2: the SOURCE
+    grid is cut into z-slabs, every rank evaluates its slab (its own grid descriptor and slab of the
+    history) at all observation points, and one all-reduce sums the partial fields.  On the one
+    GPU here the ranks' contexts run one after another and the sum is taken on the host; it must
+    equal the unsharded call and the oracle (the fields are linear in the sources, Eq. (4)-(5))."""
+    import bench
+    w = wl.random_history((10, 9, 8), 40, seed=93, dtype=dtype, n_obs=(12, 11, 6), dt=0.05)
+    ctx = make_ctx(w, jb)
+    try:
+        upload(ctx, w)
+        E, B = gpu_fields(ctx, w, 39)
+    finally:
+        ctx.close()
+    Es, Bs = np.zeros_like(E), np.zeros_like(B)
+    for r in range(world):
+        z0, z1 = bench.source_slab(w.n_src[2], r, world)
+        v = bench.slab_workload(w, z0, z1)
+        c = jb.Jefi(v.n_src, v.slab_origin, v.spacing_src, dt=w.dt, c=w.c, nsteps=w.T, dtype=w.dtype,
+                    n_obs=w.n_obs, origin_obs=w.origin_obs, spacing_obs=w.spacing_obs)
+        try:
+            upload(c, v)
+            e, b = gpu_fields(c, w, 39)
+            Es += e; Bs += b
+        finally:
+            c.close()
+    tol = tol_for(w)
+    assert max(rel_l2(Es, E, field_ref=E)) <= tol and max(rel_l2(Bs, B, field_ref=B)) <= tol
+    Eo, Bo = oracle_fields(w, 39)
+    check(w, Es, Bs, Eo, Bo, None, f"source slabs x{world} {dtype}")

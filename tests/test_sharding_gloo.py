@@ -58,6 +58,17 @@ def _worker(rank, world, port, out_dir):
         parts = [torch.zeros_like(mine) for _ in range(world)]
         dist.all_gather(parts, mine)
         full = torch.cat([p[:, :int(s)] for p, s in zip(parts, sizes)], dim=1).numpy()
+        # --scaling strong --split src: every rank evaluates ITS z-slab of the source grid (own grid
+        # descriptor, own slab of the history) at every observation point; bench.sum_partial_fields
+        # all-reduces the partial fields into the total on every rank
+        z0, z1 = bench.source_slab(w.n_src[2], rank, world)
+        v = bench.slab_workload(w, z0, z1)
+        Es, Bs = oracle.fields(v.n_src, v.slab_origin, v.spacing_src, v.rho, v.J, dt=w.dt, c=w.c, step=11,
+                               obs_xyz=w.obs_points(), nthreads=1)
+        Et, Bt = torch.from_numpy(Es.copy()), torch.from_numpy(Bs.copy())
+        bench.sum_partial_fields(Et, Bt)
+        if rank == 0:
+            np.save(os.path.join(out_dir, "src_split.npy"), np.concatenate([Et.numpy(), Bt.numpy()]))
         # the timing reduction of bench.py: every rank ends with the slowest rank's numbers
         red = bench.max_over_ranks([10.0 + rank, 5.0 - rank], device="cpu")
         if rank == 0:
@@ -82,7 +93,22 @@ def test_two_ranks_partition_the_observation_set(tmp_path):
     np.testing.assert_array_equal(full[:3], E)
     np.testing.assert_array_equal(full[3:], B)
     assert list(np.load(tmp_path / "sizes.npy")) == [36, 24]        # 3 + 2 z-layers of 4 x 3
+    # source split: the all-reduced slab fields equal the unsharded evaluation up to summation order
+    tot = np.load(tmp_path / "src_split.npy")
+    np.testing.assert_allclose(tot[:3], E, rtol=0, atol=1e-13 * np.abs(E).max())
+    np.testing.assert_allclose(tot[3:], B, rtol=0, atol=1e-13 * np.abs(B).max())
     assert list(np.load(tmp_path / "red.npy")) == [11.0, 5.0]
+
+
+def test_source_slabs_partition_the_layers():
+    import bench
+    for nz, world in ((64, 8), (48, 5), (3, 4), (100, 3)):
+        pos = 0
+        for r in range(world):
+            z0, z1 = bench.source_slab(nz, r, world)
+            assert z0 == pos and z1 >= z0
+            pos = z1
+        assert pos == nz
 
 
 @pytest.mark.parametrize("n,world", [((64, 64, 64), 8), ((256, 256, 1), 8), ((100, 100, 100), 3),
