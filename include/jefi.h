@@ -154,7 +154,8 @@ jefi_status jefi_fields(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t 
  * output steps, whose retarded steps are consecutive stored snapshots; it reads a second copy
  * of the history ("series layout": the raw 16-byte {rho, J/c} record per (cell, step), time
  * differences formed in registers), which the context allocates on the first such call
- * (N_s x (nsteps+3) x 16 B (fp32) / 32 B (fp64)) and rebuilds from the packed history after
+ * (N_s x (nsteps+3) x 16 B (fp32) / 32 B (fp64); the partial-sum scratch is regrown on that call
+ * too, to at most 1 GiB, if the series does not fit it) and rebuilds from the packed history after
  * every jefi_upload_history / jefi_append_step.  Other requests (point lists, one or two steps,
  * windows beyond shared memory) run step_count one-step evaluations.  All launches are enqueued
  * on `stream` back to back; step_count = 0 is a no-op. */

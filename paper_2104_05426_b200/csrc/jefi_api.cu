@@ -359,6 +359,27 @@ jefi_status jefi_fields_series(jefi_ctx* ctx, int32_t step_begin, int32_t step_c
             ctx->launches += n;
             ctx->series_valid = true;
         }
+        // The partial sums of a series are [chunks][steps][6][points]: when the scratch sized by
+        // jefi_create for one-step calls cannot hold the whole series twice over, it is regrown
+        // once (up to 1 GiB) so that the series goes in one batch of step blocks instead of several
+        // (X1: 411 steps x 3375 points in 3 batches of ~2 waves -> 1 batch of 5 waves).
+        {
+            const int nsb = jefi::series_block_steps(ctx->dtype);
+            long long want = 2LL * 6 * obs_count * ((step_count + nsb - 1) / nsb * nsb);
+            if (want > (1LL << 27)) want = 1LL << 27;
+            if (want > ctx->scratch_alloc_elems && ctx->scratch_elems == ctx->scratch_alloc_elems) {
+                void* bigger = nullptr;
+                if (cudaMalloc(&bigger, (size_t)want * sizeof(double)) == cudaSuccess) {
+                    cudaDeviceSynchronize();                   // earlier launches may still use the old one
+                    cudaFree(ctx->scratch);
+                    ctx->dev_bytes += (want - ctx->scratch_alloc_elems) * (long long)sizeof(double);
+                    ctx->scratch = bigger;
+                    ctx->scratch_elems = ctx->scratch_alloc_elems = want;
+                } else {
+                    cudaGetLastError();                        // no room: keep the batches
+                }
+            }
+        }
         jefi::FieldsLaunch L;
         L.step = step_begin; L.obs_begin = obs_begin; L.obs_count = obs_count;
         L.E_out = E_out_dev; L.B_out = B_out_dev;
