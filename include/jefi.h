@@ -212,6 +212,49 @@ int         jefi_flops_per_pair(void);
 jefi_status jefi_shard_obs(const jefi_obs_desc* obs, int32_t rank, int32_t world,
                            int64_t* begin, int64_t* count);
 
+/* Steps a2-a6 for callers that cannot allocate device memory.
+ *
+ * Every other entry point needs a jefi_ctx, and jefi_create cudaMallocs the packed history, the
+ * partial-sum scratch and the staging buffers.  That rules the library out for two kinds of host:
+ * a solver embedded in an application whose own memory pool has already taken all free device
+ * memory (cudaMalloc just fails there), and a stepping loop that must never stall (cudaMalloc and
+ * cudaFree synchronise the whole device).  jefi_fields_noalloc is for them: no context, and no
+ * cudaMalloc, cudaFree or allocating library routine on any path through it.
+ *
+ * Same definition and same descriptors as jefi_create + jefi_upload_history + jefi_fields (Eq.
+ * (4)-(6); screening PAPER.md:75; deriv_mode, rounding of the retarded step and
+ * powers of c as stated at the top of this file), same tolerances against it, not the same bits.
+ * The caller passes its own buffers: the raw history rho_dev[nsteps][N_s], J_dev[nsteps][3][N_s]
+ * (device, `dtype`, read only, x fastest) and the outputs E_out_dev, B_out_dev [3][obs_count]
+ * (device, `dtype`, fully overwritten); obs / obs_begin / obs_count / step as in jefi_fields;
+ * time->t0 is not used.  A per-point kernel reads the raw snapshots and differences them in
+ * time on the fly (no packed history), so it is far slower than the tiled kernels behind
+ * jefi_fields -- it is meant for modest problems, not for the benchmark configurations.
+ *
+ * Scratch: the partial sums of the source chunks go to ONE fixed array of
+ * JEFI_NOALLOC_SCRATCH_BYTES that is part of the library image; each GPU that loads libjefi.so
+ * holds it until the process exits, used or not.  Hence the limit: obs_count larger than
+ * JEFI_NOALLOC_MAX_OBS is refused with JEFI_ERR_UNSUPPORTED and a message saying so (split the
+ * request into several calls, or use a context); N_s and nsteps are not limited.  All calls on
+ * a device share that array: calls whose kernels may overlap on the GPU (two streams, no
+ * ordering between them) race on it and give wrong fields; issue them on one stream or order
+ * them with events.  A call never depends on what an earlier call left there.
+ *
+ * Works on the CURRENT device (cudaSetDevice is the caller's business; all pointers must belong
+ * to it) and enqueues two kernels on `stream` without waiting for them.  The first call on each
+ * device also does a one-time set-up (it asks the runtime where that device keeps the scratch
+ * array); make that first call outside any stream capture.  Thread-safe as far as that set-up
+ * goes.  `err` (host, may be NULL) receives a NUL-terminated message of at most err_len bytes on
+ * failure and "" on success.  Arguments are checked before any CUDA call. */
+#define JEFI_NOALLOC_SCRATCH_BYTES (8 * 1024 * 1024)
+#define JEFI_NOALLOC_MAX_OBS       131072
+jefi_status jefi_fields_noalloc(const jefi_grid_desc* src, const jefi_obs_desc* obs,
+                                const jefi_time_desc* time, jefi_dtype dtype, int32_t step,
+                                const void* rho_dev, const void* J_dev,
+                                int64_t obs_begin, int64_t obs_count,
+                                void* E_out_dev, void* B_out_dev, jefi_stream stream,
+                                char* err, int32_t err_len);
+
 #ifdef __cplusplus
 }
 #endif

@@ -25,7 +25,9 @@ EXPORTS = (                                   # include/jefi.h: the product ABI
     "jefi_device_bytes", "jefi_destroy", "jefi_status_string", "jefi_last_error",
     "jefi_flops_per_pair", "jefi_shard_obs",
     "jefi_append_step", "jefi_append_step_host", "jefi_fields_series", "jefi_fields_series_host",
+    "jefi_fields_noalloc",
 )
+JEFI_NOALLOC_SCRATCH_BYTES, JEFI_NOALLOC_MAX_OBS = 8 * 1024 * 1024, 131072
 INSTRUMENT_EXPORTS = (                        # include/jefi_instrument.h: bench / test instrumentation
     "jefi_launch_count", "jefi_measure_alu_peak", "jefi_measure_ffma_operand_rates", "jefi_debug_pair_lags", "jefi_debug_launch_limits",
 )
@@ -71,6 +73,9 @@ _lib.jefi_fields_series_host.argtypes = [_P, C.c_int32, C.c_int32, C.c_int64, C.
 _lib.jefi_fields_at_time.argtypes = [_P, C.c_double, C.c_int64, C.c_int64, _P, _P, _P]
 _lib.jefi_fields_host.argtypes = [_P, C.c_int32, C.c_int64, C.c_int64, _P, _P, _P]
 _lib.jefi_set_kernel.argtypes = [_P, C.c_int32]
+_lib.jefi_fields_noalloc.argtypes = [C.POINTER(jefi_grid_desc), C.POINTER(jefi_obs_desc), C.POINTER(jefi_time_desc),
+                                     C.c_int, C.c_int32, _P, _P, C.c_int64, C.c_int64, _P, _P, _P, C.c_char_p,
+                                     C.c_int32]
 _lib.jefi_launch_count.argtypes = [_P]
 _lib.jefi_launch_count.restype = C.c_int64
 _lib.jefi_device_bytes.argtypes = [_P]
@@ -189,6 +194,23 @@ def jefi_fields_at_time(ctx, t, obs_begin, obs_count, E_out_dev, B_out_dev, stre
 def jefi_fields_host(ctx, step, obs_begin, obs_count, E_out_host, B_out_host, stream=None):
     _check(_lib.jefi_fields_host(ctx, int(step), int(obs_begin), int(obs_count), _ptr(E_out_host),
                                  _ptr(B_out_host), _stream(stream)), ctx, "jefi_fields_host")
+
+
+def jefi_fields_noalloc(src: jefi_grid_desc, obs: jefi_obs_desc, time: jefi_time_desc, dtype: int, step: int,
+                        rho_dev, J_dev, obs_begin, obs_count, E_out_dev, B_out_dev, stream=None):
+    """E, B of one step on the current device without a context and without any device
+    allocation (for hosts that cannot cudaMalloc: all memory already pooled by the application,
+    or a loop that must not stall).  The caller passes the raw history and the outputs; at most
+    JEFI_NOALLOC_MAX_OBS points per call; calls that overlap on the GPU race on the library's
+    one fixed scratch array.  See include/jefi.h."""
+    msg = C.create_string_buffer(512)
+    st = _lib.jefi_fields_noalloc(C.byref(src) if src is not None else None,
+                                  C.byref(obs) if obs is not None else None,
+                                  C.byref(time) if time is not None else None, int(dtype), int(step),
+                                  _ptr(rho_dev), _ptr(J_dev), int(obs_begin), int(obs_count), _ptr(E_out_dev),
+                                  _ptr(B_out_dev), _stream(stream), msg, len(msg))
+    if st != JEFI_OK:
+        raise JefiError(st, "jefi_fields_noalloc", msg.value.decode())
 
 
 def jefi_set_kernel(ctx, which: int):
