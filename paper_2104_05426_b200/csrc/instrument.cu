@@ -105,7 +105,8 @@ double run_operand(int sm_count)
 
 // ------------------------------------------------------------------ lag dump
 struct LagArgs {
-    int nsx, nsy, nox, noy;
+    int nsx, nsy, nsz, nox, noy;
+    float tie_lim_list;         // the list kernel's near-tie threshold (pairwise_list.cu), 0 = no list tiling
     double shx, shy, shz, ohx, ohy, ohz, d0x, d0y, d0z, sox, soy, soz;
     double rcut2, inv_cdt;
     int obs_kind, which;
@@ -124,25 +125,44 @@ lag_dump_kernel(const long long* __restrict__ obs_idx, const long long* __restri
     const long long gi = obs_idx[t], j = cell_idx[t];
     const int jx = (int)(j % a.nsx), jy = (int)((j / a.nsx) % a.nsy), jz = (int)(j / ((long long)a.nsx * a.nsy));
     T ox, oy, oz;
+    double pdx = 0, pdy = 0, pdz = 0;
     if (a.obs_kind == 0) {
         const int ix = (int)(gi % a.nox), iy = (int)((gi / a.nox) % a.noy);
         const int iz = (int)(gi / ((long long)a.nox * a.noy));
         ox = obs_coord<T>(a.d0x, ix, a.ohx); oy = obs_coord<T>(a.d0y, iy, a.ohy); oz = obs_coord<T>(a.d0z, iz, a.ohz);
     } else {
         const T* p = (const T*)a.points + 3 * gi;
-        ox = (T)((double)p[0] - a.sox); oy = (T)((double)p[1] - a.soy); oz = (T)((double)p[2] - a.soz);
+        pdx = (double)p[0] - a.sox; pdy = (double)p[1] - a.soy; pdz = (double)p[2] - a.soz;
+        ox = (T)pdx; oy = (T)pdy; oz = (T)pdz;
     }
+    // fp32 on a point list: the kernels redo near-tie lags in fp64 (tiled_common.cuh tie_delta,
+    // near_tie_lag); the same test with the same threshold each of them uses
+    const bool fix_ties = sizeof(T) == 4 && a.obs_kind == 1;
     T dy, dz, dx, w;
     const T ryz = row_ryz<T>(oy, oz, jy, jz, (T)a.shy, (T)a.shz, dy, dz);
     int k;
     if (a.which == 1) {
         point_geo<T>(ox, jx, (T)a.shx, ryz, (T)a.rcut2, -tie_biased_neg_inv_cdt<T>(a.inv_cdt), dx, w, k);
+        if (fix_ties) {
+            const double fx = fmax(fabs(pdx), fabs(pdx - (a.nsx - 1) * a.shx));
+            const double fy = fmax(fabs(pdy), fabs(pdy - (a.nsy - 1) * a.shy));
+            const double fz = fmax(fabs(pdz), fabs(pdz - (a.nsz - 1) * a.shz));
+            const T tie_lim = (T)(0.5f - tie_delta(sqrt(fx * fx + fy * fy + fz * fz) * a.inv_cdt));
+            const T e = (dx * dx + ryz) * w * (T)a.inv_cdt - (T)k;
+            if ((e < T(0) ? -e : e) >= tie_lim && w != T(0))
+                k = near_tie_lag(pdx, pdy, pdz, jx, jy, jz, a.shx, a.shy, a.shz, a.inv_cdt);
+        }
     } else {
         unsigned bits;
+        T R;
         // (the SLOW variant: the one the kernels run wherever a pair can be as close as R = 0, and
         // identical to the fast one for every R2 >= 1e-30)
-        pair_geo<T, true>(ox, src_coord<T>(jx, a.shx), ryz, tie_biased_neg_inv_cdt<T>(a.inv_cdt), (T)a.rcut2, dx, w, bits);
+        pair_geo_r<T, true>(ox, src_coord<T>(jx, a.shx), ryz, tie_biased_neg_inv_cdt<T>(a.inv_cdt), (T)a.rcut2, dx, w, bits, R);
         k = lag_of_bits(bits, Prec<T>::kMagicLo);
+        if (fix_ties) {
+            const float e = fmaf((float)R, (float)(-a.inv_cdt), (float)k);
+            if (fabsf(e) >= a.tie_lim_list) k = near_tie_lag(pdx, pdy, pdz, jx, jy, jz, a.shx, a.shy, a.shz, a.inv_cdt);
+        }
     }
     out[t] = k;
 }
@@ -186,10 +206,11 @@ jefi_status jefi_debug_pair_lags(jefi_ctx* ctx, int32_t which, int64_t n_pairs, 
     if (n_pairs == 0) return JEFI_OK;
     if (!obs_index_dev || !cell_index_dev || !lag_out_dev) return JEFI_ERR_INVALID_ARG;
     const jefi::Params& P = ctx->P;
-    if (which == 2 && P.obs_kind != 0) return JEFI_ERR_UNSUPPORTED;
+    if (which == 2 && P.obs_kind != 0 && !ctx->tiles.perm) return JEFI_ERR_UNSUPPORTED;
     if (cudaSetDevice(ctx->device) != cudaSuccess) { cudaGetLastError(); return JEFI_ERR_CUDA; }
     jefi::LagArgs a;
-    a.nsx = P.ns[0]; a.nsy = P.ns[1]; a.nox = P.no[0]; a.noy = P.no[1];
+    a.nsx = P.ns[0]; a.nsy = P.ns[1]; a.nsz = P.ns[2]; a.nox = P.no[0]; a.noy = P.no[1];
+    a.tie_lim_list = P.obs_kind != 0 && ctx->tiles.perm ? 0.5f - jefi::tie_delta(ctx->tiles.far / (P.c * P.dt)) : 0.f;
     a.shx = P.sh[0]; a.shy = P.sh[1]; a.shz = P.sh[2];
     a.ohx = P.oh[0]; a.ohy = P.oh[1]; a.ohz = P.oh[2];
     a.d0x = P.oo[0] - P.so[0]; a.d0y = P.oo[1] - P.so[1]; a.d0z = P.oo[2] - P.so[2];

@@ -178,7 +178,60 @@ struct ListArgs {
     int wcap_rt, chunk_base, accumulate, flush_stages;
     int wmax, stages, stage_bytes, cps;
     const void* points; const int* perm; const double* boxes;
+    float tie_lim;                            // fp32: |q - k| >= tie_lim is "near a tie" (0.5 - tie_delta)
 };
+
+// fp32 near-tie pairs (tiled_common.cuh tie_delta): the few pairs whose q is within the fp32
+// error of a half-integer take their lag from fp64 coordinate differences, as the contract's
+// k = floor(q + 1/2) is defined (include/jefi.h).  The hot loop stays branch-free: it adds every
+// pair with its fp32 lag and only MARKS the near-tie ones (three instructions and a predicated OR
+// into a per-point bit mask, one bit per cell of the row segment); after the segment the marked
+// pairs -- 4e-4 of all on the c3 geometry -- are revisited: fp64 lag (out of line, fed from seven
+// doubles thread 0 parks in the unused bytes [160, 216) of the shared-memory map of
+// tiled_step.cuh), and where it differs from the fp32 one (about one marked pair in four) the
+// pair's terms are taken out again and added with the record of the right step.  (A branch
+// around the pair inside the unrolled loop cost 48 % on c3_points: it stops the compiler from
+// overlapping the gathers of neighbouring pairs.)
+constexpr unsigned kOffTie = 160;
+__device__ __noinline__ unsigned list_tie_bits(const double* tc, const float* p, int jx, int jy, int jz)
+{
+    const int k = near_tie_lag((double)p[0] - tc[0], (double)p[1] - tc[1], (double)p[2] - tc[2], jx, jy, jz, tc[3], tc[4],
+                               tc[5], tc[6]);
+    return Prec<float>::kMagicLo - (unsigned)k;
+}
+template <bool SLOW>
+__device__ __forceinline__ void pair_update_mark(Acc<float>& a, float ox, float ryz, const CellMeta<float>& m,
+                                                 float neg_inv_cdt, float rcut2, int n1, unsigned unit_off,
+                                                 float neg_inv_plain, float tie_lim, unsigned& mask, unsigned bit)
+{
+    float dx, w, R;
+    unsigned bits;
+    pair_geo_r<float, SLOW>(ox, m.sx, ryz, neg_inv_cdt, rcut2, dx, w, bits, R);
+    // bits = magic - k as a float pattern: e = k - q (without the tie bias), |e| <= 1/2
+    const float e = fmaf(R, neg_inv_plain, 12582912.0f - __uint_as_float(bits));
+    if (fabsf(e) >= tie_lim) mask |= bit;
+    pair_accumulate<float>(a, dx, w, record_addr<float, SLOW>(m, bits, n1), unit_off);
+}
+// the marked pairs of one point over one row segment (cells jx0.. of row jy, jz; meta at meta_addr)
+__device__ __forceinline__ void fix_marked_pairs(Acc<float>& a, unsigned mask, float ox, float ryz, unsigned meta_addr,
+                                                 bool slow_stage, float neg_inv_cdt, float rcut2, int n1, unsigned unit_off,
+                                                 const double* tc, const float* p, int jx0, int jy, int jz)
+{
+    while (mask) {
+        const int c = __ffs(mask) - 1;
+        mask &= mask - 1;
+        const CellMeta<float> m = load_meta(meta_addr + c * 16u, 0.f);
+        float dx, w, R;
+        unsigned bits;
+        pair_geo_r<float, true>(ox, m.sx, ryz, neg_inv_cdt, rcut2, dx, w, bits, R);     // as in the hot loop
+        const unsigned good = list_tie_bits(tc, p, jx0 + c, jy, jz);
+        if (good == bits || w == 0.f) continue;
+        const unsigned was = slow_stage ? record_addr<float, true>(m, bits, n1) : record_addr<float, false>(m, bits, n1);
+        const unsigned now = slow_stage ? record_addr<float, true>(m, good, n1) : record_addr<float, false>(m, good, n1);
+        pair_accumulate<float, true>(a, dx, w, was, unit_off);
+        pair_accumulate<float, false>(a, dx, w, now, unit_off);
+    }
+}
 
 template <typename T, int WCAP, int CW, int CTAS>
 __global__ void __launch_bounds__((CW + 1) * 32, CTAS)
@@ -201,6 +254,8 @@ fields_list_kernel(const uint4* __restrict__ hist, double* __restrict__ partial,
             mbar_init(sbase + kOffEmpty + 8 * s, CW);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        double* tc = reinterpret_cast<double*>(smem + kOffTie);
+        tc[0] = a.sox; tc[1] = a.soy; tc[2] = a.soz; tc[3] = a.shx; tc[4] = a.shy; tc[5] = a.shz; tc[6] = a.inv_cdt;
     }
     __syncthreads();
 
@@ -277,7 +332,8 @@ fields_list_kernel(const uint4* __restrict__ hist, double* __restrict__ partial,
     // point i of thread tid = entry tile*TP + i*(32 CW) + tid of the sorted order; entries past the
     // end of the list compute a copy of the last point and store nothing
     T ox[P], oy[P], oz[P];
-    long long gi[P];
+    int gi[P];                                  // caller's index of the point (perm is int)
+    unsigned okmask = 0;                        // bit i: entry i is a real point (stored at the end)
     Acc<T> acc[P];
     const T* pts = (const T*)a.points;
 #pragma unroll
@@ -285,15 +341,21 @@ fields_list_kernel(const uint4* __restrict__ hist, double* __restrict__ partial,
         long long s = (long long)tile * TP + i * (CW * 32) + tid;
         const bool ok = s < a.n_points;
         s = ok ? s : a.n_points - 1;
-        const long long g = a.perm[s];
-        gi[i] = ok ? g : -1;
-        ox[i] = (T)((double)pts[3 * g + 0] - a.sox);
-        oy[i] = (T)((double)pts[3 * g + 1] - a.soy);
-        oz[i] = (T)((double)pts[3 * g + 2] - a.soz);
+        const int g = a.perm[s];
+        gi[i] = g;
+        okmask |= ok ? 1u << i : 0u;
+        ox[i] = (T)((double)pts[3 * (long long)g + 0] - a.sox);
+        oy[i] = (T)((double)pts[3 * (long long)g + 1] - a.soy);
+        oz[i] = (T)((double)pts[3 * (long long)g + 2] - a.soz);
         acc[i] = Acc<T>{0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
     }
     const T shy = (T)a.shy, shz = (T)a.shz, rcut2 = (T)a.rcut2;
     const T neg_inv_cdt = tie_biased_neg_inv_cdt<T>(a.inv_cdt);
+    const float neg_inv_plain = (float)(-a.inv_cdt), tie_lim = a.tie_lim;
+    unsigned tmask[P];                          // fp32: bit c = pair (point i, cell c of the row segment) is near a tie
+#pragma unroll
+    for (int i = 0; i < P; ++i) tmask[i] = 0;
+    const double* tc = reinterpret_cast<const double*>(smem + kOffTie);
     int jx = (int)(cb % a.nsx), jy = (int)((cb / a.nsx) % a.nsy), jz = (int)(cb / ((long long)a.nsx * a.nsy));
     int since = 0;
     bool first = a.accumulate == 0;
@@ -317,14 +379,39 @@ fields_list_kernel(const uint4* __restrict__ hist, double* __restrict__ partial,
                 for (int c = 0; c < len; ++c) {
                     const CellMeta<T> m = load_meta(meta_addr + c * 16u, T(0));
 #pragma unroll
-                    for (int i = 0; i < P; ++i) pair_update<T, true>(acc[i], ox[i], ryz[i], m, neg_inv_cdt, rcut2, a.n1, unit_off);
+                    for (int i = 0; i < P; ++i) {
+                        if constexpr (sizeof(T) == 4)
+                            pair_update_mark<true>(acc[i], ox[i], ryz[i], m, neg_inv_cdt, rcut2, a.n1, unit_off, neg_inv_plain,
+                                                   tie_lim, tmask[i], 1u << c);
+                        else
+                            pair_update<T, true>(acc[i], ox[i], ryz[i], m, neg_inv_cdt, rcut2, a.n1, unit_off);
+                    }
                 }
             } else {
 #pragma unroll 4
                 for (int c = 0; c < len; ++c) {
                     const CellMeta<T> m = load_meta(meta_addr + c * 16u, T(0));
 #pragma unroll
-                    for (int i = 0; i < P; ++i) pair_update<T, false>(acc[i], ox[i], ryz[i], m, neg_inv_cdt, rcut2, a.n1, unit_off);
+                    for (int i = 0; i < P; ++i) {
+                        if constexpr (sizeof(T) == 4)
+                            pair_update_mark<false>(acc[i], ox[i], ryz[i], m, neg_inv_cdt, rcut2, a.n1, unit_off, neg_inv_plain,
+                                                    tie_lim, tmask[i], 1u << c);
+                        else
+                            pair_update<T, false>(acc[i], ox[i], ryz[i], m, neg_inv_cdt, rcut2, a.n1, unit_off);
+                    }
+                }
+            }
+            if constexpr (sizeof(T) == 4) {
+                unsigned any = 0;
+#pragma unroll
+                for (int i = 0; i < P; ++i) any |= tmask[i];
+                if (any) {
+#pragma unroll
+                    for (int i = 0; i < P; ++i) {
+                        fix_marked_pairs(acc[i], tmask[i], ox[i], ryz[i], meta_addr, slow != 0, neg_inv_cdt, rcut2, a.n1,
+                                         unit_off, tc, (const float*)pts + 3 * (long long)gi[i], jx, jy, jz);
+                        tmask[i] = 0;
+                    }
                 }
             }
             pos += len; jx += len;
@@ -342,7 +429,7 @@ fields_list_kernel(const uint4* __restrict__ hist, double* __restrict__ partial,
             since = 0;
 #pragma unroll
             for (int i = 0; i < P; ++i) {
-                if (gi[i] >= 0) {
+                if (okmask >> i & 1u) {
                     double* out = partial + (long long)blockIdx.y * 6 * a.obs_count + gi[i];
                     const T v[6] = {acc[i].ex, acc[i].ey, acc[i].ez, acc[i].bx, acc[i].by, acc[i].bz};
 #pragma unroll
@@ -377,8 +464,9 @@ int launch_list_cap(const Params& P, jefi_dtype dt, const void* hist, const Fiel
     a.points = P.obs_points; a.perm = pt.perm; a.boxes = pt.boxes;
 
     const double wd = floor(pt.max_diam * a.inv_cdt) + 5.0;
-    if (wd > 1.0e6 || pt.far * a.inv_cdt > 2.0e6) return 0;
+    if (wd > 1.0e6 || pt.far * a.inv_cdt > kMaxLagSteps) return 0;
     a.wmax = (int)wd;
+    a.tie_lim = 0.5f - tie_delta(pt.far * a.inv_cdt);
     if (WCAP > 0 && a.wmax > WCAP) return 0;
     const int wcap = WCAP > 0 ? WCAP : (a.wmax + 7) / 8 * 8;
     a.wcap_rt = wcap;

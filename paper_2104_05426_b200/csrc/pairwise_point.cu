@@ -57,14 +57,27 @@ fields_point_kernel(const T* __restrict__ hist, double* __restrict__ partial, Po
 
     // observation position relative to the centre of source cell (0,0,0)
     T ox, oy, oz;
+    double pdx = 0, pdy = 0, pdz = 0;       // the same in fp64 (point lists in fp32: near-tie lags)
     if (a.obs_kind == 0) {
         const int ix = (int)(gi % a.nox), iy = (int)((gi / a.nox) % a.noy);
         const int iz = (int)(gi / ((long long)a.nox * a.noy));
         ox = obs_coord<T>(a.d0x, ix, a.ohx); oy = obs_coord<T>(a.d0y, iy, a.ohy); oz = obs_coord<T>(a.d0z, iz, a.ohz);
     } else {
         const T* p = (const T*)a.points + 3 * gi;
-        ox = (T)((double)p[0] - a.sox); oy = (T)((double)p[1] - a.soy); oz = (T)((double)p[2] - a.soz);
+        pdx = (double)p[0] - a.sox; pdy = (double)p[1] - a.soy; pdz = (double)p[2] - a.soz;
+        ox = (T)pdx; oy = (T)pdy; oz = (T)pdz;
     }
+    // fp32 on an explicit point list: pairs whose q is within tie_delta of a half-integer get
+    // their lag from fp64 (tiled_common.cuh near_tie_lag); grids keep the lattice arithmetic
+    const bool fix_ties = sizeof(T) == 4 && a.obs_kind == 1;
+    float tie_lim = 0.f;
+    if (fix_ties) {
+        const double fx = fmax(fabs(pdx), fabs(pdx - (a.nsx - 1) * a.shx));
+        const double fy = fmax(fabs(pdy), fabs(pdy - (a.nsy - 1) * a.shy));
+        const double fz = fmax(fabs(pdz), fabs(pdz - (a.nsz - 1) * a.shz));
+        tie_lim = 0.5f - tie_delta(sqrt(fx * fx + fy * fy + fz * fz) * a.inv_cdt);
+    }
+    const T inv_cdt_plain = (T)a.inv_cdt;
     const T shx = (T)a.shx, shy = (T)a.shy, shz = (T)a.shz;
     const T rcut2 = (T)a.rcut2, inv_cdt = -tie_biased_neg_inv_cdt<T>(a.inv_cdt);
 
@@ -87,6 +100,11 @@ fields_point_kernel(const T* __restrict__ hist, double* __restrict__ partial, Po
             T dx, rinv;
             int k;
             point_geo<T>(ox, sx, shx, ryz, rcut2, inv_cdt, dx, rinv, k);
+            if (fix_ties) {
+                const T e = (dx * dx + ryz) * rinv * inv_cdt_plain - (T)k;      // q - k in [-1/2, 1/2]
+                if ((e < T(0) ? -e : e) >= (T)tie_lim && rinv != T(0))
+                    k = near_tie_lag(pdx, pdy, pdz, sx, sy, sz, a.shx, a.shy, a.shz, a.inv_cdt);
+            }
             int p = a.n1 - k;
             p = p < 0 ? 0 : p;
             const Rec<T> h = load_rec(hist, j, a.Tp, ring_slot(p, a.origin, a.Tp - 1));      // rho, rho', Jx, Jy, Jz, Jx', Jy', Jz'

@@ -485,7 +485,7 @@ int launch_series_shape(const Params& P, jefi_dtype dt, const void* series, cons
     const double far = sqrt(pow(fabs(a.d0x) + ex + P.no[0] * P.oh[0] + P.ns[0] * P.sh[0], 2) +
                             pow(fabs(a.d0y) + ey + P.no[1] * P.oh[1] + P.ns[1] * P.sh[1], 2) +
                             pow(fabs(a.d0z) + ez + P.no[2] * P.oh[2] + P.ns[2] * P.sh[2], 2));
-    if (far * a.inv_cdt > 2.0e6) return 0;
+    if (far * a.inv_cdt > kMaxLagSteps) return 0;
     a.wcap = ((int)wd + 7) / 8 * 8;
 
     const int cell_bytes = U * a.wcap * 16;

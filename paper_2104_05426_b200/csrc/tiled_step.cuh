@@ -44,29 +44,32 @@ template <typename T> struct Acc {
     T s, ux, uy, uz, vy, vz;      // per source row
 };
 
+// shared-memory address of the record a pair reads: fast path straight from the lag bits, slow
+// path (stages that may hold p <= 0 or screened pairs) through the clamped packed step
 template <typename T, bool SLOW>
-__device__ __forceinline__ void pair_update(Acc<T>& a, T ox, T ryz, const CellMeta<T>& m, T neg_inv_cdt, T rcut2, int n1,
-                                            unsigned unit_off)
+__device__ __forceinline__ unsigned record_addr(const CellMeta<T>& m, unsigned bits, int n1)
 {
-    T dx, w;
-    unsigned bits;
-    pair_geo<T, SLOW>(ox, m.sx, ryz, neg_inv_cdt, rcut2, dx, w, bits);
-    unsigned addr;
     if (SLOW) {
         int p = n1 - lag_of_bits(bits, Prec<T>::kMagicLo);
         p = p < 0 ? 0 : p;
-        addr = m.C2 + ((unsigned)p << 4);
-    } else {
-        addr = m.C + (bits << 4);
+        return m.C2 + ((unsigned)p << 4);
     }
+    return m.C + (bits << 4);
+}
+// gather the record and add the pair's terms to the running sums (NEG: take them out again --
+// every term is a product with g, h or w, so negating those three negates the pair)
+template <typename T, bool NEG = false>
+__device__ __forceinline__ void pair_accumulate(Acc<T>& a, T dx, T w, unsigned addr, unsigned unit_off)
+{
     T v[8];
     load_record(addr, unit_off, v);
-    const T g = w * w;
-    const T h = dx * g;
+    T g = w * w;
+    T h = dx * g;
     const T ts = fma_t<T>(v[0], w, v[1]);
     const T tx = fma_t<T>(v[2], w, v[5]);
     const T ty = fma_t<T>(v[3], w, v[6]);
     const T tz = fma_t<T>(v[4], w, v[7]);
+    if (NEG) { g = -g; h = -h; w = -w; }
     a.ex = fma_t<T>(ts, h, a.ex);
     a.s  = fma_t<T>(ts, g, a.s);
     a.ex = fma_t<T>(-v[5], w, a.ex);
@@ -77,6 +80,16 @@ __device__ __forceinline__ void pair_update(Acc<T>& a, T ox, T ryz, const CellMe
     a.uz = fma_t<T>(tz, g, a.uz);
     a.vy = fma_t<T>(ty, h, a.vy);
     a.vz = fma_t<T>(tz, h, a.vz);
+}
+
+template <typename T, bool SLOW>
+__device__ __forceinline__ void pair_update(Acc<T>& a, T ox, T ryz, const CellMeta<T>& m, T neg_inv_cdt, T rcut2, int n1,
+                                            unsigned unit_off)
+{
+    T dx, w;
+    unsigned bits;
+    pair_geo<T, SLOW>(ox, m.sx, ryz, neg_inv_cdt, rcut2, dx, w, bits);
+    pair_accumulate<T>(a, dx, w, record_addr<T, SLOW>(m, bits, n1), unit_off);
 }
 
 template <typename T>

@@ -268,12 +268,11 @@ def test_point_list_at_c3_scale_and_degenerate_sets(jb):
     """65 536 unstructured points on a 64^3 x 221-step history (fp32; the geometry of the bench
     workload c3_points): the oracle on 8192 seeded points, every other output against the
     per-point kernel.  Two histories.  (a) Smooth in time (the collision snapshot of step 190
-    modulated by 1 + 0.3 sin): both kernels must meet the fp32 bar.  (b) The collision history
-    itself, whose Lorentz-contracted discs sweep a cell in two steps: with ~1e-4 of the 1.7e10
-    pairs inside the fp32 error of a lag tie (unstructured geometry, q up to 220) no fp32
-    evaluation can reproduce the fp64 oracle's nearest-snapshot choices -- stated limitation,
-    DESIGN.md Q3; the error is measured, printed and bounded at 2e-2, and the two kernels must
-    still agree with each other as closely as they do with the oracle.  Then the degenerate sets:
+    modulated by 1 + 0.3 sin).  (b) The collision history itself, whose Lorentz-contracted discs
+    sweep a cell in two steps: ~1e-4 of the 1.7e10 pairs lie within the fp32 error of a lag tie
+    (unstructured geometry, q up to 220), where one flipped lag is an O(1) error in that term; the
+    fp32 list kernels find those pairs and take their lag in fp64 (Q3 (ii)), so both
+    histories must meet the fp32 bar of north_star in both kernels.  Then the degenerate sets:
     all points identical (one bin, zero-size boxes), points on a line, a single point."""
     for smooth in (True, False):
         w = wl.config3_collision()
@@ -290,19 +289,14 @@ def test_point_list_at_c3_scale_and_degenerate_sets(jb):
                 ctx.set_kernel(kernel)
                 E, B = gpu_fields(ctx, w, 220)
                 out[kernel] = (E, B)
-                if smooth:
-                    check(w, E[:, idx], B[:, idx], Eo, Bo, None, f"c3-scale points, smooth history, kernel {kernel}")
-                else:
-                    eE = max(rel_l2(E[:, idx], Eo, field_ref=Eo)); eB = max(rel_l2(B[:, idx], Bo, field_ref=Bo))
-                    print(f"\nc3 collision history, 65536 unstructured points, fp32 kernel {kernel} vs fp64 oracle: "
-                          f"rel-L2 E {eE:.2e} B {eB:.2e} (near-tie lag choices)")
-                    assert eE < 2e-2 and eB < 2e-2
+                eE, eB = check(w, E[:, idx], B[:, idx], Eo, Bo, None,
+                               f"c3-scale points, {'smooth' if smooth else 'collision'} history, kernel {kernel}")
+                print(f"\nc3 {'smooth' if smooth else 'collision'} history, 65536 unstructured points, fp32 kernel "
+                      f"{kernel} vs fp64 oracle: rel-L2 E {max(eE):.2e} B {max(eB):.2e}")
             for a, b, name in ((out[2][0], out[1][0], "E"), (out[2][1], out[1][1], "B")):
-                lim = 4e-4 if smooth else 2e-2
-                assert max(rel_l2(a, b, field_ref=b)) <= lim, name
-                if smooth:
-                    rms = np.sqrt(np.mean(np.sum(b * b, axis=0)))
-                    assert np.abs(a - b).max() <= 4e-3 * rms, name
+                assert max(rel_l2(a, b, field_ref=b)) <= 4e-4, name
+                rms = np.sqrt(np.mean(np.sum(b * b, axis=0)))
+                assert np.abs(a - b).max() <= 4e-3 * rms, name
         finally:
             ctx.close()
     w = wl.random_history((6, 5, 4), 24, seed=15, dtype="f64", dt=0.05)
@@ -737,7 +731,8 @@ def test_fuzz_random_lattices_fp32(jb):
             idx = np.arange(begin, begin + count)
             Eo, Bo = oracle_fields(w, step, idx, mode)
             check(w, E, B, Eo, Bo, None, f"fp32 fuzz {ran}: src {n_src} obs {n_obs} T {T} step {step} "
-                                          f"range {begin}+{count} mode {mode} dx/cdt {ratio}")
+                                          f"range {begin}+{count} mode {mode} dx/cdt {ratio}",
+                  comp_floor=1e-3)        # DESIGN.md Q10: the same floor as the fp32 series fuzz
             ran += 1
         finally:
             ctx.close()
@@ -812,6 +807,37 @@ def test_retarded_index_mismatch_count_is_zero_on_every_config(jb, name, dtype):
             bad = np.nonzero(kg != ko)[0]
             assert bad.size == 0, (f"{name} {dtype} kernel {which}: {bad.size} of {len(ko)} lags differ, e.g. pair "
                                    f"(obs {obs[bad[0]]}, cell {cell[bad[0]]}): kernel {kg[bad[0]]} oracle {ko[bad[0]]}")
+    finally:
+        ctx.close()
+
+
+def test_near_tie_lags_on_unstructured_points_equal_the_oracle_in_fp32(jb):
+    """DESIGN.md Q3 (ii): on the 65 536 seeded points over the c3 source grid, the pairs whose
+    q = R/(c dt) lies within 1e-3 of a half-integer (picked from 8 million seeded pairs; numpy is
+    used only to PICK them) plus 30 000 unselected pairs: the lag of both fp32 list kernels
+    (per-point and tiled, near-tie pairs redone in fp64) must equal the oracle's on every one."""
+    w = wl.with_random_points(_geometry("c3", "f32"), 65536)
+    n = 8_000_000
+    u = wl.uniform01(w.seed + 77, 0, 2 * n)
+    obs = np.minimum((u[:n] * w.N_o).astype(np.int64), w.N_o - 1)
+    cell = np.minimum((u[n:] * w.N_s).astype(np.int64), w.N_s - 1)
+    nx, ny, nz = w.n_src
+    src = np.stack([w.origin_src[0] + (cell % nx) * w.spacing_src[0],
+                    w.origin_src[1] + ((cell // nx) % ny) * w.spacing_src[1],
+                    w.origin_src[2] + (cell // (nx * ny)) * w.spacing_src[2]], axis=1)
+    q = np.linalg.norm(w.points[obs] - src, axis=1) / (w.c * w.dt)
+    near = np.nonzero(np.abs(q - np.floor(q) - 0.5) < 1e-3)[0]
+    assert near.size > 10000, near.size
+    pick = np.concatenate([near, np.arange(30000)])
+    obs, cell = obs[pick], cell[pick]
+    ko = _oracle_lags(w, obs, cell)
+    ctx = make_ctx(w, jb)
+    try:
+        for which in (1, 2):
+            kg = _kernel_lags(jb, ctx, which, obs, cell)
+            bad = np.nonzero(kg != ko)[0]
+            assert bad.size == 0, (f"kernel {which}: {bad.size} of {len(ko)} lags differ, e.g. pair (obs {obs[bad[0]]}, "
+                                   f"cell {cell[bad[0]]}): kernel {kg[bad[0]]} oracle {ko[bad[0]]}, q {q[pick][bad[0]]!r}")
     finally:
         ctx.close()
 
@@ -1004,7 +1030,7 @@ def test_source_slabs_sum_to_the_full_evaluation(jb, world, dtype):
     history) at all observation points, and one all-reduce sums the partial fields.  On the one
     GPU here the ranks' contexts run one after another and the sum is taken on the host; it must
     equal the unsharded call and the oracle (the fields are linear in the sources, Eq. (4)-(5))."""
-    import bench
+    from paper_2104_05426_b200 import sharding
     w = wl.random_history((10, 9, 8), 40, seed=93, dtype=dtype, n_obs=(12, 11, 6), dt=0.05)
     ctx = make_ctx(w, jb)
     try:
@@ -1014,9 +1040,9 @@ def test_source_slabs_sum_to_the_full_evaluation(jb, world, dtype):
         ctx.close()
     Es, Bs = np.zeros_like(E), np.zeros_like(B)
     for r in range(world):
-        z0, z1 = bench.source_slab(w.n_src[2], r, world)
-        v = bench.slab_workload(w, z0, z1)
-        c = jb.Jefi(v.n_src, v.slab_origin, v.spacing_src, dt=w.dt, c=w.c, nsteps=w.T, dtype=w.dtype,
+        z0, z1, slab_origin, _ = sharding.src_slab(w.n_src, w.origin_src, w.spacing_src, r, world)
+        v = wl.slab_workload(w, z0, z1)
+        c = jb.Jefi(v.n_src, slab_origin, v.spacing_src, dt=w.dt, c=w.c, nsteps=w.T, dtype=w.dtype,
                     n_obs=w.n_obs, origin_obs=w.origin_obs, spacing_obs=w.spacing_obs)
         try:
             upload(c, v)
