@@ -87,8 +87,9 @@ typedef struct {
     int32_t past_mode;
 } jefi_time_desc;
 
-/* Validates the descriptors, selects `device`, and allocates everything the context will
- * ever need on it: the packed history (32 bytes (fp32) / 64 bytes (fp64) per (cell, step), plus
+/* Validates the descriptors, selects `device`, and allocates what the one-step calls need on
+ * it (the series calls and the *_host uploads add their own buffers on first use, see there and
+ * jefi_reserve_series): the packed history (32 bytes (fp32) / 64 bytes (fp64) per (cell, step), plus
  * one all-zero step standing for m < 0), the raw values of the two newest steps (for
  * jefi_append_step), partial-sum scratch, and the device output staging used by
  * jefi_fields_host.  For a regular observation grid no kernel is launched; for a point list
@@ -156,7 +157,11 @@ jefi_status jefi_fields(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t 
  * differences formed in registers), which the context allocates on the first such call
  * (N_s x (nsteps+3) x 16 B (fp32) / 32 B (fp64); the partial-sum scratch is regrown on that call
  * too, to at most 1 GiB, if the series does not fit it) and rebuilds from the packed history after
- * every jefi_upload_history / jefi_append_step.  Other requests (point lists, one or two steps,
+ * every jefi_upload_history / jefi_append_step.  One known difference from step_count one-step
+ * calls: after a jefi_append_step the rebuilt series layout differences the OLDEST stored step
+ * one-sided from the stored values ((f[1] - f[0])/dt in centred mode, f[0]/dt in backward mode),
+ * whereas the packed record of that step keeps the derivative it had before the append (see
+ * jefi_append_step); only pairs whose retarded step is that oldest step are affected.  Other requests (point lists, one or two steps,
  * windows beyond shared memory) run step_count one-step evaluations.  All launches are enqueued
  * on `stream` back to back; step_count = 0 is a no-op. */
 jefi_status jefi_fields_series(jefi_ctx* ctx, int32_t step_begin, int32_t step_count,
@@ -169,6 +174,19 @@ jefi_status jefi_fields_series(jefi_ctx* ctx, int32_t step_begin, int32_t step_c
 jefi_status jefi_fields_series_host(jefi_ctx* ctx, int32_t step_begin, int32_t step_count,
                                     int64_t obs_begin, int64_t obs_count,
                                     void* E_out_host, void* B_out_host, jefi_stream stream);
+
+/* The series calls above allocate on first use (series layout, a larger partial-sum scratch, the
+ * host path's staging), and growing a buffer that earlier launches may still read waits for the
+ * whole device (cudaDeviceSynchronize) before freeing it -- so the FIRST series call of a size is
+ * not a pure enqueue.  A stepping loop that must stay asynchronous calls jefi_reserve_series once
+ * beforehand: it makes those allocations for series of up to max_steps steps on up to max_obs
+ * points (host_staging != 0: also the staging of jefi_fields_series_host).  Afterwards
+ * jefi_fields_series[_host] within those limits call no cudaMalloc / cudaFree /
+ * cudaDeviceSynchronize and jefi_device_bytes stays constant.  Synchronous; may be called again
+ * with larger limits (buffers only grow); JEFI_ERR_INVALID_ARG unless 1 <= max_steps <= nsteps and
+ * 1 <= max_obs <= N_o; JEFI_ERR_OOM if the layout or the staging does not fit (a scratch that
+ * cannot be regrown is not an error: the series then runs in several batches). */
+jefi_status jefi_reserve_series(jefi_ctx* ctx, int32_t max_steps, int64_t max_obs, int32_t host_staging);
 
 /* Same for a time t that must lie on the step grid to within 1e-6*dt (the paper
  * evaluates at snapshots only), else JEFI_ERR_TIME_RANGE. */
@@ -211,6 +229,20 @@ int         jefi_flops_per_pair(void);
  * JEFI_ERR_INVALID_ARG on null pointers, world <= 0 or rank outside [0, world). */
 jefi_status jefi_shard_obs(const jefi_obs_desc* obs, int32_t rank, int32_t world,
                            int64_t* begin, int64_t* count);
+
+/* The other decomposition of the paper's Fig. 2: the SOURCE region is cut
+ * and every rank evaluates the fields of its own sources at every observation point; the fields
+ * are linear in rho and J (Eq. (4)-(5)), so one sum over the ranks (an all-reduce of the 6 N_o
+ * values) gives the total.  Host-only helper: rank `rank` of `world` owns a contiguous run of
+ * whole z-layers of `src` (sizes differ by at most one layer); *slab is the grid descriptor of
+ * that run -- the same x, y extent and spacing, n[2] = its layers, origin[2] moved to its first
+ * layer -- to be given to jefi_create as the source grid, and *cell_begin the linear index of its
+ * first cell in the full grid: the rank's history is rows [cell_begin, cell_begin + slab cells) of
+ * every rho[m][.] and J[m][comp][.].  A rank beyond the number of layers gets n[2] = 0 (nothing
+ * to do; not a grid jefi_create accepts).  JEFI_ERR_INVALID_ARG on null pointers, a bad grid,
+ * world <= 0 or rank outside [0, world).  Touches no device. */
+jefi_status jefi_shard_src(const jefi_grid_desc* src, int32_t rank, int32_t world,
+                           jefi_grid_desc* slab, int64_t* cell_begin);
 
 /* Steps a2-a6 for callers that cannot allocate device memory.
  *

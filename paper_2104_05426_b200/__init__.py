@@ -25,7 +25,7 @@ EXPORTS = (                                   # include/jefi.h: the product ABI
     "jefi_device_bytes", "jefi_destroy", "jefi_status_string", "jefi_last_error",
     "jefi_flops_per_pair", "jefi_shard_obs",
     "jefi_append_step", "jefi_append_step_host", "jefi_fields_series", "jefi_fields_series_host",
-    "jefi_fields_noalloc",
+    "jefi_fields_noalloc", "jefi_reserve_series", "jefi_shard_src",
 )
 JEFI_NOALLOC_SCRATCH_BYTES, JEFI_NOALLOC_MAX_OBS = 8 * 1024 * 1024, 131072
 INSTRUMENT_EXPORTS = (                        # include/jefi_instrument.h: bench / test instrumentation
@@ -73,6 +73,7 @@ _lib.jefi_fields_series_host.argtypes = [_P, C.c_int32, C.c_int32, C.c_int64, C.
 _lib.jefi_fields_at_time.argtypes = [_P, C.c_double, C.c_int64, C.c_int64, _P, _P, _P]
 _lib.jefi_fields_host.argtypes = [_P, C.c_int32, C.c_int64, C.c_int64, _P, _P, _P]
 _lib.jefi_set_kernel.argtypes = [_P, C.c_int32]
+_lib.jefi_reserve_series.argtypes = [_P, C.c_int32, C.c_int64, C.c_int32]
 _lib.jefi_fields_noalloc.argtypes = [C.POINTER(jefi_grid_desc), C.POINTER(jefi_obs_desc), C.POINTER(jefi_time_desc),
                                      C.c_int, C.c_int32, _P, _P, C.c_int64, C.c_int64, _P, _P, _P, C.c_char_p,
                                      C.c_int32]
@@ -88,6 +89,8 @@ _lib.jefi_last_error.restype = C.c_char_p
 _lib.jefi_flops_per_pair.argtypes = []
 _lib.jefi_measure_alu_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
 _lib.jefi_shard_obs.argtypes = [C.POINTER(jefi_obs_desc), C.c_int32, C.c_int32, C.POINTER(C.c_int64),
+                                C.POINTER(C.c_int64)]
+_lib.jefi_shard_src.argtypes = [C.POINTER(jefi_grid_desc), C.c_int32, C.c_int32, C.POINTER(jefi_grid_desc),
                                 C.POINTER(C.c_int64)]
 _lib.jefi_measure_ffma_operand_rates.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
 _lib.jefi_debug_pair_lags.argtypes = [_P, C.c_int32, C.c_int64, _P, _P, _P, _P]
@@ -186,6 +189,11 @@ def jefi_fields_series_host(ctx, step_begin, step_count, obs_begin, obs_count, E
            "jefi_fields_series_host")
 
 
+def jefi_reserve_series(ctx, max_steps, max_obs, host_staging=False):
+    _check(_lib.jefi_reserve_series(ctx, int(max_steps), int(max_obs), 1 if host_staging else 0), ctx,
+           "jefi_reserve_series")
+
+
 def jefi_fields_at_time(ctx, t, obs_begin, obs_count, E_out_dev, B_out_dev, stream=None):
     _check(_lib.jefi_fields_at_time(ctx, float(t), int(obs_begin), int(obs_count), _ptr(E_out_dev),
                                     _ptr(B_out_dev), _stream(stream)), ctx, "jefi_fields_at_time")
@@ -267,6 +275,16 @@ def jefi_shard_obs(obs: jefi_obs_desc, rank: int, world: int):
     return b.value, n.value
 
 
+def jefi_shard_src(src: jefi_grid_desc, rank: int, world: int):
+    """(slab descriptor, cell_begin) of the source z-layers rank `rank` of `world` owns."""
+    slab, cb = jefi_grid_desc(), C.c_int64()
+    st = _lib.jefi_shard_src(C.byref(src) if src is not None else None, int(rank), int(world), C.byref(slab),
+                             C.byref(cb))
+    if st != JEFI_OK:
+        raise JefiError(st, "jefi_shard_src")
+    return slab, cb.value
+
+
 def make_obs_grid(n, origin, spacing) -> jefi_obs_desc:
     obs = jefi_obs_desc()
     obs.kind = 0
@@ -323,6 +341,9 @@ class Jefi:
                            stream=None):
         n = self.n_points - obs_begin if obs_count is None else obs_count
         jefi_fields_series_host(self.ctx, step_begin, step_count, obs_begin, n, E_out_host, B_out_host, stream)
+
+    def reserve_series(self, max_steps, max_obs=None, host_staging=False):
+        jefi_reserve_series(self.ctx, max_steps, self.n_points if max_obs is None else max_obs, host_staging)
 
     def fields_host(self, step, E_out_host, B_out_host, obs_begin=0, obs_count=None, stream=None):
         n = self.n_points - obs_begin if obs_count is None else obs_count

@@ -102,9 +102,68 @@ jefi_status run_fields(jefi_ctx* ctx, int32_t step, int64_t obs_begin, int64_t o
     return JEFI_OK;
 }
 
+// The partial sums of a series are [chunks][steps][6][points]: when the scratch sized by
+// jefi_create for one-step calls cannot hold the whole series twice over, it is regrown (up to
+// 1 GiB) so that the series goes in one batch of step blocks instead of several.  Blocks the
+// device when it grows; never shrinks; keeps the old scratch if there is no room.
+void grow_series_scratch(jefi_ctx* ctx, long long step_count, long long obs_count)
+{
+    const int nsb = jefi::series_block_steps(ctx->dtype);
+    long long want = 2LL * 6 * obs_count * ((step_count + nsb - 1) / nsb * nsb);
+    if (want > (1LL << 27)) want = 1LL << 27;
+    if (want <= ctx->scratch_alloc_elems || ctx->scratch_elems != ctx->scratch_alloc_elems) return;
+    void* bigger = nullptr;
+    if (cudaMalloc(&bigger, (size_t)want * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return; }
+    cudaDeviceSynchronize();                   // earlier launches may still use the old one
+    cudaFree(ctx->scratch);
+    ctx->dev_bytes += (want - ctx->scratch_alloc_elems) * (long long)sizeof(double);
+    ctx->scratch = bigger;
+    ctx->scratch_elems = ctx->scratch_alloc_elems = want;
+}
+
+// device staging of jefi_fields_series_host (E then B); growing frees the old one, so it waits
+// for the copies still reading it
+jefi_status grow_series_staging(jefi_ctx* ctx, size_t bytes)
+{
+    if (ctx->stage_series_bytes >= bytes) return JEFI_OK;
+    if (ctx->stage_series) { cudaDeviceSynchronize(); cudaFree(ctx->stage_series); ctx->dev_bytes -= (long long)ctx->stage_series_bytes; }
+    ctx->stage_series = nullptr; ctx->stage_series_bytes = 0;
+    jefi_status s = dev_alloc(ctx, &ctx->stage_series, bytes, "cudaMalloc(series staging)");
+    if (s == JEFI_OK) ctx->stage_series_bytes = bytes;
+    return s;
+}
+
+jefi_status alloc_series_layout(jefi_ctx* ctx)
+{
+    if (ctx->series) return JEFI_OK;
+    const size_t bytes = (size_t)ctx->P.Ns * (size_t)(ctx->P.T + 3) * 4 * ctx->elem;
+    ctx->series_valid = false;
+    return dev_alloc(ctx, &ctx->series, bytes, "cudaMalloc(series layout)");
+}
+
 }  // namespace
 
 extern "C" {
+
+jefi_status jefi_reserve_series(jefi_ctx* ctx, int32_t max_steps, int64_t max_obs, int32_t host_staging)
+{
+    if (!ctx) return JEFI_ERR_INVALID_ARG;
+    ctx->err[0] = 0;
+    if (max_steps <= 0 || max_steps > ctx->P.T || max_obs <= 0 || max_obs > ctx->P.n_obs) {
+        set_err(ctx, "jefi_reserve_series: max_steps must be in [1, nsteps], max_obs in [1, N_o]", cudaSuccess);
+        return JEFI_ERR_INVALID_ARG;
+    }
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e != cudaSuccess) return cuda_fail(ctx, "cudaSetDevice", e);
+    jefi_status s = alloc_series_layout(ctx);
+    if (s != JEFI_OK) return s;
+    grow_series_scratch(ctx, max_steps, max_obs);
+    if (host_staging) {
+        s = grow_series_staging(ctx, 2 * (size_t)max_steps * 3 * (size_t)max_obs * ctx->elem);
+        if (s != JEFI_OK) return s;
+    }
+    return JEFI_OK;
+}
 
 jefi_status jefi_create(const jefi_grid_desc* src, const jefi_obs_desc* obs,
                         const jefi_time_desc* time, jefi_dtype dtype, int device, jefi_ctx** out)
@@ -348,11 +407,7 @@ jefi_status jefi_fields_series(jefi_ctx* ctx, int32_t step_begin, int32_t step_c
     if ((ctx->kernel_choice == 0 || ctx->kernel_choice == 3) && ctx->P.obs_kind == 0 && 2 * step_count >= jefi::series_block_steps(ctx->dtype)) {
         cudaError_t e = cudaSetDevice(ctx->device);
         if (e != cudaSuccess) return cuda_fail(ctx, "cudaSetDevice", e);
-        if (!ctx->series) {
-            const size_t bytes = (size_t)ctx->P.Ns * (size_t)(ctx->P.T + 3) * 4 * ctx->elem;
-            if ((s = dev_alloc(ctx, &ctx->series, bytes, "cudaMalloc(series layout)")) != JEFI_OK) return s;
-            ctx->series_valid = false;
-        }
+        if ((s = alloc_series_layout(ctx)) != JEFI_OK) return s;
         if (!ctx->series_valid) {
             int n = jefi::launch_series_layout(ctx->P, ctx->dtype, ctx->hist, ctx->series, (cudaStream_t)stream);
             if (n < 0) return cuda_fail(ctx, "series layout launch", cudaGetLastError());
@@ -363,23 +418,7 @@ jefi_status jefi_fields_series(jefi_ctx* ctx, int32_t step_begin, int32_t step_c
         // jefi_create for one-step calls cannot hold the whole series twice over, it is regrown
         // once (up to 1 GiB) so that the series goes in one batch of step blocks instead of several
         // (X1: 411 steps x 3375 points in 3 batches of ~2 waves -> 1 batch of 5 waves).
-        {
-            const int nsb = jefi::series_block_steps(ctx->dtype);
-            long long want = 2LL * 6 * obs_count * ((step_count + nsb - 1) / nsb * nsb);
-            if (want > (1LL << 27)) want = 1LL << 27;
-            if (want > ctx->scratch_alloc_elems && ctx->scratch_elems == ctx->scratch_alloc_elems) {
-                void* bigger = nullptr;
-                if (cudaMalloc(&bigger, (size_t)want * sizeof(double)) == cudaSuccess) {
-                    cudaDeviceSynchronize();                   // earlier launches may still use the old one
-                    cudaFree(ctx->scratch);
-                    ctx->dev_bytes += (want - ctx->scratch_alloc_elems) * (long long)sizeof(double);
-                    ctx->scratch = bigger;
-                    ctx->scratch_elems = ctx->scratch_alloc_elems = want;
-                } else {
-                    cudaGetLastError();                        // no room: keep the batches
-                }
-            }
-        }
+        grow_series_scratch(ctx, step_count, obs_count);
         jefi::FieldsLaunch L;
         L.step = step_begin; L.obs_begin = obs_begin; L.obs_count = obs_count;
         L.E_out = E_out_dev; L.B_out = B_out_dev;
@@ -442,17 +481,15 @@ jefi_status jefi_fields_series_host(jefi_ctx* ctx, int32_t step_begin, int32_t s
     if (step_count == 0) return JEFI_OK;
     jefi_status s = check_fields_args(ctx, step_begin, obs_begin, obs_count, E_out_host, B_out_host);
     if (s != JEFI_OK) return s;
+    if (step_count > ctx->P.T - step_begin) {          // before anything is sized from step_count
+        set_err(ctx, "step outside the stored history", cudaSuccess);
+        return JEFI_ERR_TIME_RANGE;
+    }
     if (obs_count == 0) return JEFI_OK;
     cudaError_t e = cudaSetDevice(ctx->device);
     if (e != cudaSuccess) return cuda_fail(ctx, "cudaSetDevice", e);
     const size_t half = (size_t)step_count * 3 * (size_t)obs_count * ctx->elem;
-    if (ctx->stage_series_bytes < 2 * half) {
-        // (growing frees the old staging: wait for the copies still reading it)
-        if (ctx->stage_series) { cudaDeviceSynchronize(); cudaFree(ctx->stage_series); ctx->dev_bytes -= (long long)ctx->stage_series_bytes; }
-        ctx->stage_series = nullptr; ctx->stage_series_bytes = 0;
-        if ((s = dev_alloc(ctx, &ctx->stage_series, 2 * half, "cudaMalloc(series staging)")) != JEFI_OK) return s;
-        ctx->stage_series_bytes = 2 * half;
-    }
+    if ((s = grow_series_staging(ctx, 2 * half)) != JEFI_OK) return s;
     char* Ed = (char*)ctx->stage_series;
     char* Bd = Ed + half;
     s = jefi_fields_series(ctx, step_begin, step_count, obs_begin, obs_count, Ed, Bd, stream);
@@ -524,6 +561,20 @@ jefi_status jefi_shard_obs(const jefi_obs_desc* obs, int32_t rank, int32_t world
     const int64_t units = total / granule, base = units / world, rem = units % world;
     *begin = (rank * base + (rank < rem ? rank : rem)) * granule;
     *count = (base + (rank < rem ? 1 : 0)) * granule;
+    return JEFI_OK;
+}
+
+jefi_status jefi_shard_src(const jefi_grid_desc* src, int32_t rank, int32_t world, jefi_grid_desc* slab,
+                           int64_t* cell_begin)
+{
+    if (!src || !slab || !cell_begin || world <= 0 || rank < 0 || rank >= world) return JEFI_ERR_INVALID_ARG;
+    if (!grid_ok(*src)) return JEFI_ERR_INVALID_ARG;
+    const int64_t nz = src->n[2], base = nz / world, rem = nz % world;
+    const int64_t z0 = rank * base + (rank < rem ? rank : rem), nl = base + (rank < rem ? 1 : 0);
+    *slab = *src;
+    slab->n[2] = (int32_t)nl;
+    slab->origin[2] = src->origin[2] + (double)z0 * src->spacing[2];
+    *cell_begin = z0 * (int64_t)src->n[0] * (int64_t)src->n[1];
     return JEFI_OK;
 }
 

@@ -145,6 +145,8 @@ def test_series_and_instrument_entry_points_reject_null_arguments(jb):
     assert lib.jefi_launch_count(None) == 0
     lib.jefi_set_kernel.argtypes = [P, C.c_int32]
     assert lib.jefi_set_kernel(None, 3) == jb.JEFI_ERR_INVALID_ARG
+    lib.jefi_reserve_series.argtypes = [P, C.c_int32, C.c_int64, C.c_int32]
+    assert lib.jefi_reserve_series(None, 1, 1, 0) == jb.JEFI_ERR_INVALID_ARG
 
 
 def test_create_rejects_a_point_list_without_positions(jb):

@@ -154,6 +154,46 @@ def test_series_matches_single_step_calls_and_errors(jb):
         ctx.close()
 
 
+def test_reserve_series_makes_the_series_calls_allocation_free(jb):
+    """include/jefi.h: after jefi_reserve_series the series entry points within the reserved limits
+    neither allocate nor free (jefi_device_bytes, which counts every buffer of the context, is constant),
+    and the results are those of an unreserved context.  Without the reserve call the first series
+    call grows the context (the documented lazy behaviour)."""
+    import torch
+    w = wl.random_history((9, 8, 7), 48, seed=77, dtype="f32", n_obs=(12, 11, 10), dt=0.05)
+    ref_ctx = make_ctx(w, jb)
+    ctx = make_ctx(w, jb)
+    try:
+        upload(ref_ctx, w)
+        upload(ctx, w)
+        before = jb.jefi_device_bytes(ref_ctx.ctx)
+        Er, Br = gpu_fields_series(ref_ctx, w, 0, 48)
+        assert jb.jefi_device_bytes(ref_ctx.ctx) > before            # lazy: layout (+ scratch) on first use
+
+        with pytest.raises(jb.JefiError) as e:
+            ctx.reserve_series(49)
+        assert e.value.status == jb.JEFI_ERR_INVALID_ARG
+        ctx.reserve_series(48, host_staging=True)
+        reserved = jb.jefi_device_bytes(ctx.ctx)
+        assert reserved > before
+        E = torch.empty((48, 3, w.N_o), dtype=torch.float32, device="cuda")
+        B = torch.empty_like(E)
+        Eh = torch.empty((48, 3, w.N_o), dtype=torch.float32).pin_memory()
+        Bh = torch.empty_like(Eh).pin_memory()
+        ctx.fields_series(0, 48, E, B)
+        ctx.fields_series(5, 17, E, B, 100, 333)
+        ctx.fields_series_host(0, 48, Eh, Bh)
+        torch.cuda.synchronize()
+        assert jb.jefi_device_bytes(ctx.ctx) == reserved
+        np.testing.assert_array_equal(Eh.numpy().astype(np.float64), Er)
+        np.testing.assert_array_equal(Bh.numpy().astype(np.float64), Br)
+        ctx.reserve_series(10, 5)                                     # smaller limits: nothing shrinks or grows
+        assert jb.jefi_device_bytes(ctx.ctx) == reserved
+    finally:
+        ctx.close()
+        ref_ctx.close()
+
+
 # ------------------------------------------------------------------ config 4, all 128 output steps
 def test_series_config4_all_128_steps(jb):
     """BASELINE.json configs[3]: the 128-step time series of the detached plane in ONE call,

@@ -28,6 +28,7 @@ def _worker(rank, world, port, out_dir):
     import torch.distributed as dist
     import oracle
     import paper_2104_05426_b200 as jb
+    from paper_2104_05426_b200 import sharding
     import bench
 
     os.environ["MASTER_ADDR"] = "127.0.0.1"
@@ -35,14 +36,15 @@ def _worker(rank, world, port, out_dir):
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
         w = wl.random_history((5, 4, 3), 12, seed=3, dtype="f64", n_obs=(4, 3, 5), dt=0.05)
-        # bench.py --scaling strong, host side: only rank 0 holds the raw history; the others
-        # receive it through bench.broadcast_history, then every rank evaluates ITS slice of the
-        # one observation set (bench.strong_slice -> jefi_shard_obs)
+        # observation split (paper_2104_05426_b200/sharding.py, what bench.py --scaling strong runs):
+        # only rank 0 holds the raw history; the others receive it through broadcast_history, then
+        # every rank evaluates ITS slice of the one observation set (obs_slice -> jefi_shard_obs)
         rho = torch.from_numpy(w.rho.copy()) if rank == 0 else torch.zeros(w.rho.shape, dtype=torch.float64)
         J = torch.from_numpy(w.J.copy()) if rank == 0 else torch.zeros(w.J.shape, dtype=torch.float64)
-        bench.broadcast_history(rho, J)
+        sharding.broadcast_history(rho, J)
         assert np.array_equal(rho.numpy(), w.rho) and np.array_equal(J.numpy(), w.J)
-        begin, count = bench.strong_slice(jb, w, rank, world)
+        begin, count = sharding.obs_slice(w.n_obs, w.origin_obs, w.spacing_obs, rank=rank, world=world)
+        assert (begin, count) == bench.strong_slice(jb, w, rank, world)
         obs = jb.make_obs_grid(w.n_obs, w.origin_obs, w.spacing_obs)
         assert (begin, count) == jb.jefi_shard_obs(obs, rank, world)
         idx = np.arange(begin, begin + count)
@@ -58,15 +60,16 @@ def _worker(rank, world, port, out_dir):
         parts = [torch.zeros_like(mine) for _ in range(world)]
         dist.all_gather(parts, mine)
         full = torch.cat([p[:, :int(s)] for p, s in zip(parts, sizes)], dim=1).numpy()
-        # --scaling strong --split src: every rank evaluates ITS z-slab of the source grid (own grid
-        # descriptor, own slab of the history) at every observation point; bench.sum_partial_fields
+        # source split: every rank evaluates ITS z-slab of the source grid (own grid descriptor from
+        # jefi_shard_src, own slab of the history) at every observation point; sum_partial_fields
         # all-reduces the partial fields into the total on every rank
-        z0, z1 = bench.source_slab(w.n_src[2], rank, world)
-        v = bench.slab_workload(w, z0, z1)
+        z0, z1, slab_origin, cell_begin = sharding.src_slab(w.n_src, w.origin_src, w.spacing_src, rank, world)
+        v = wl.slab_workload(w, z0, z1)
+        assert v.slab_origin == pytest.approx(slab_origin) and cell_begin == z0 * w.n_src[0] * w.n_src[1]
         Es, Bs = oracle.fields(v.n_src, v.slab_origin, v.spacing_src, v.rho, v.J, dt=w.dt, c=w.c, step=11,
                                obs_xyz=w.obs_points(), nthreads=1)
         Et, Bt = torch.from_numpy(Es.copy()), torch.from_numpy(Bs.copy())
-        bench.sum_partial_fields(Et, Bt)
+        sharding.sum_partial_fields(Et, Bt)
         if rank == 0:
             np.save(os.path.join(out_dir, "src_split.npy"), np.concatenate([Et.numpy(), Bt.numpy()]))
         # the timing reduction of bench.py: every rank ends with the slowest rank's numbers
@@ -101,14 +104,29 @@ def test_two_ranks_partition_the_observation_set(tmp_path):
 
 
 def test_source_slabs_partition_the_layers():
-    import bench
-    for nz, world in ((64, 8), (48, 5), (3, 4), (100, 3)):
-        pos = 0
+    """jefi_shard_src: contiguous whole z-layers in rank order, sizes within one layer of each
+    other, slab descriptors that tile the source grid exactly; bad arguments are refused."""
+    import __graft_entry__
+    __graft_entry__.build()
+    import paper_2104_05426_b200 as jb
+    for n, world in (((64, 64, 64), 8), ((48, 48, 48), 5), ((7, 5, 3), 4), ((100, 100, 100), 3), ((4, 3, 1), 2)):
+        src = jb.make_grid(n, (-1.5, 0.25, 2.0), (0.1, 0.2, 0.3))
+        pos, sizes = 0, []
         for r in range(world):
-            z0, z1 = bench.source_slab(nz, r, world)
-            assert z0 == pos and z1 >= z0
-            pos = z1
-        assert pos == nz
+            slab, cell_begin = jb.jefi_shard_src(src, r, world)
+            assert cell_begin == pos * n[0] * n[1]
+            assert list(slab.n)[:2] == list(n[:2]) and list(slab.spacing) == [0.1, 0.2, 0.3]
+            assert list(slab.origin)[:2] == [-1.5, 0.25] and slab.origin[2] == pytest.approx(2.0 + pos * 0.3)
+            pos += slab.n[2]
+            sizes.append(slab.n[2])
+        assert pos == n[2] and max(sizes) - min(sizes) <= 1 and sizes == sorted(sizes, reverse=True)
+    src = jb.make_grid((4, 4, 4), (0, 0, 0), (1, 1, 1))
+    for rank, world in ((0, 0), (-1, 2), (2, 2)):
+        with pytest.raises(jb.JefiError) as e:
+            jb.jefi_shard_src(src, rank, world)
+        assert e.value.status == jb.JEFI_ERR_INVALID_ARG
+    with pytest.raises(jb.JefiError):
+        jb.jefi_shard_src(None, 0, 1)
 
 
 @pytest.mark.parametrize("n,world", [((64, 64, 64), 8), ((256, 256, 1), 8), ((100, 100, 100), 3),

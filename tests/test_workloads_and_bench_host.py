@@ -54,7 +54,7 @@ def test_bench_descriptors():
     assert "obs-sharded x8" in bench.config_dict(w, "c3_small", 8, "strong")["parallelism"]
     assert "z-slabs x8" in bench.config_dict(w, "c3_small", 8, "strong-src")["parallelism"]
     assert bench.is_series("c4_series") and bench.is_series("c4_series_f64") and not bench.is_series("c4")
-    v = bench.slab_workload(w, 3, 7)
+    v = wl.slab_workload(w, 3, 7)
     assert v.n_src == (16, 16, 4) and v.rho.shape[1] == 4 and v.J.shape[2] == 4
     assert v.slab_origin[2] == pytest.approx(w.origin_src[2] + 3 * w.spacing_src[2])
     np.testing.assert_array_equal(v.rho, w.rho[:, 3:7])

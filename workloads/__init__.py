@@ -348,3 +348,17 @@ def smooth_in_time(w: Workload, period: float, depth: float = 0.3, base_step: in
     w.J = np.ascontiguousarray((w.J[base_step].astype(np.float64)[None] * f[:, None]).astype(w.np_dtype))
     w.name = f"{w.name}_smooth{period:g}"
     return w
+
+
+def slab_workload(w: Workload, z0: int, z1: int) -> Workload:
+    """The workload restricted to source layers [z0, z1) (a rank's share when the SOURCE region is
+    partitioned): its own grid size, ``slab_origin`` = the centre of its cell
+    (0,0,0), and its own slab of the history; observation set unchanged.  Slicing only."""
+    import copy
+    v = copy.copy(w)
+    v.n_src = (w.n_src[0], w.n_src[1], z1 - z0)
+    o = w.origin_src
+    v.slab_origin = (o[0], o[1], o[2] + z0 * w.spacing_src[2])
+    v.rho = np.ascontiguousarray(w.rho[:, z0:z1])
+    v.J = np.ascontiguousarray(w.J[:, :, z0:z1])
+    return v
