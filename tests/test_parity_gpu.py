@@ -98,6 +98,35 @@ def test_config3_collision_full_size_sampled(jb, kernel):
     run_case(jb, w, w.obs_subset(16384), kernel)        # 16 384 seeded points, 4.3e9 pairs
 
 
+def test_config3_world8_observation_slices_concatenate_to_the_full_result(jb):
+    """SURVEY.md 8(e) on c3's real shape: jefi_shard_obs cuts the 64 z-layers of observation points
+    into 8 slices of 8 layers (one tile layer each); evaluated one after another on the one GPU
+    here, their concatenation in rank order must equal the unsharded call within the fp32 bar (the
+    launcher picks a different source-chunk count per slice, so the summation order differs) and
+    meet the oracle on the seeded sample."""
+    w = wl.config3_collision()
+    obs = jb.make_obs_grid(w.n_obs, w.origin_obs, w.spacing_obs)
+    ctx = make_ctx(w, jb)
+    try:
+        upload(ctx, w)
+        E, B = gpu_fields(ctx, w, w.steps[-1])
+        parts, pos = [], 0
+        for r in range(8):
+            b, c = jb.jefi_shard_obs(obs, r, 8)
+            assert b == pos and c == 8 * 64 * 64
+            pos += c
+            parts.append(gpu_fields(ctx, w, w.steps[-1], b, c))
+        Ec = np.concatenate([p[0] for p in parts], axis=1)
+        Bc = np.concatenate([p[1] for p in parts], axis=1)
+        tol = tol_for(w)
+        assert max(rel_l2(Ec, E, field_ref=E)) <= tol and max(rel_l2(Bc, B, field_ref=B)) <= tol
+        idx = w.obs_subset(16384)
+        Eo, Bo = oracle_fields(w, w.steps[-1], idx)          # cached from the test above
+        check(w, Ec[:, idx], Bc[:, idx], Eo, Bo, None, "c3 in 8 observation slices")
+    finally:
+        ctx.close()
+
+
 # ------------------------------------------------------------------ config 4
 _C4_PLAN = {}
 
